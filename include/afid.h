@@ -1,0 +1,112 @@
+/*
+ * afid.h -- C ABI of the B200-native AFiD pressure-correction (projection) step.
+ *
+ * What the library computes (paper = arXiv 1705.01423, "P:L<n>" = line n of PAPER.md):
+ * one projection of a provisional, non-solenoidal velocity (u*, v*, w*) onto the discretely
+ * divergence-free fields of a staggered, conservative, second-order finite-difference grid
+ * (Fig. 1) by the fractional-step method: solve the Poisson equation
+ * D G phi = D u* for the pressure correction phi, then u = u* - G phi.  The solve
+ * is the direct method of P:L99-L114: Fourier transforms in the two periodic directions
+ * (y, z) with modified wavenumbers, one tridiagonal system in the wall-normal direction x
+ * per (ky, kz) mode, inverse transforms.  Readings of everything the paper leaves open
+ * (metrics, the singular mean mode, p = phi) are listed in DESIGN.md, section "Readings".
+ *
+ * Grid.  nx cells in x between the walls xc[0] and xc[nx] (xc: nx+1 strictly increasing
+ * face coordinates, possibly stretched); ny, nz uniform periodic cells over lengths
+ * Ly, Lz.  Arrays are C-ordered [i][j][k], k (z) fastest, fp64, 64-bit indexing:
+ *   u : (nx+1)*ny*nz  wall-normal velocity on x-faces (planes 0 and nx are the walls)
+ *   v :  nx   *ny*nz  y-velocity on y-faces
+ *   w :  nx   *ny*nz  z-velocity on z-faces
+ *   p :  nx   *ny*nz  pressure correction phi at cell centres (output only)
+ *
+ * All work runs in hand-written sm_100a CUDA kernels; there is no CPU or library (cuFFT)
+ * fallback: an unsupported size or a missing device is an error.
+ *
+ * Threading: a plan may be used by one host thread / one stream at a time.  Functions never
+ * synchronise the device unless stated.
+ */
+#ifndef AFID_H_
+#define AFID_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct afid_plan afid_plan; /* opaque; owned by the library */
+
+/* Error codes (negative).  afid_last_error() returns a message for the calling thread. */
+#define AFID_OK 0
+#define AFID_ERR_NULL (-1)             /* a required pointer is NULL                               */
+#define AFID_ERR_ALIGN (-2)            /* a device pointer is not 16-byte aligned                  */
+#define AFID_ERR_UNSUPPORTED_SIZE (-3) /* nx, ny or nz outside what the kernels are built for     */
+#define AFID_ERR_GRID (-4)             /* xc not finite / not strictly increasing, or Ly, Lz <= 0  */
+#define AFID_ERR_NOMEM (-5)            /* device or host allocation failed                         */
+#define AFID_ERR_CUDA (-6)             /* a CUDA runtime call or kernel launch failed              */
+
+/*
+ * afid_plan_create -- build a plan for an nx x ny x nz grid on the CURRENT CUDA device.
+ *   nx      cells in x, 2 <= nx <= afid_max_nx()
+ *   ny, nz  periodic cells; ny and nz/2 must be lengths the FFT kernels are instantiated
+ *           for (afid_fft_length_supported): powers of two times 1 or 3, 8..4096
+ *   xc      HOST pointer, nx+1 face coordinates (copied; caller keeps ownership)
+ *   Ly, Lz  periodic box lengths (> 0)
+ * The plan owns: reciprocal metrics, tridiagonal coefficients a_i, c_i, modified
+ * wavenumbers 2(1-cos(2 pi k/n))/Delta^2, twiddle tables, and two device work
+ * arrays of nx*ny*(nz/2+1) complex doubles each.  Synchronous (allocates and uploads).
+ * Returns NULL on failure (see afid_last_error / afid_last_error_code).
+ */
+afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly, double Lz);
+
+/*
+ * afid_project -- enqueue one projection step on `stream` (a cudaStream_t, may be NULL for
+ * the legacy default stream).  u, v, w, p are DEVICE pointers, 16-byte aligned, laid out as
+ * above, owned by the caller.  u, v, w are updated in place (the two wall planes of u are
+ * read, never written: Neumann condition on phi); p is overwritten with phi, whose
+ * dx-weighted mean is zero.  Steps (paper step numbers):
+ *   1  divergence                        3+5  forward transforms in z then y
+ *   7  tridiagonal solves in x           9+11 inverse transforms in y then z
+ *   correction u -= G phi, p = phi
+ * (steps 2,4,6,8,10,12, the pencil transposes, are folded into the kernels' tile loads).
+ * Returns AFID_OK or a negative code.  Validation is synchronous; the kernels are only
+ * enqueued, so execution errors surface at the caller's next synchronisation.
+ * NaN/Inf in the inputs propagate.  The compatibility condition (zero net wall flux) is
+ * not checked; it holds identically when u vanishes on both wall planes.
+ */
+int afid_project(afid_plan* plan, double* u, double* v, double* w, double* p, void* stream);
+
+/* afid_plan_destroy -- free the plan's device and host memory.  NULL is a no-op.
+ * The caller must have synchronised any stream still using the plan. */
+int afid_plan_destroy(afid_plan* plan);
+
+/* Device bytes held by the plan (work arrays + tables). */
+size_t afid_plan_workspace_bytes(const afid_plan* plan);
+
+/* Number of kernel launches one afid_project call enqueues (for launch accounting). */
+int afid_plan_num_launches(const afid_plan* plan);
+
+/*
+ * Stage taps, for stage-wise parity tests (same kernels as afid_project, run separately):
+ *   afid_stage_forward:  u,v,w -> spectrum of -(div u)/(ny*nz), written to `spec`
+ *                        (DEVICE, nx*(nz/2+1)*ny complex doubles, layout [i][kz][ky]).
+ *   afid_stage_solve:    spec ([i][kz][ky], in place) <- solution of the x-systems.
+ * Both enqueue on `stream` and use the plan's work arrays.
+ */
+int afid_stage_forward(afid_plan* plan, const double* u, const double* v, const double* w,
+                       double* spec, void* stream);
+int afid_stage_solve(afid_plan* plan, double* spec, void* stream);
+
+/* 1 if the FFT kernels are instantiated for complex length n (ny must satisfy this, and nz/2). */
+int afid_fft_length_supported(int n);
+/* Largest nx the tridiagonal kernel supports. */
+int afid_max_nx(void);
+
+const char* afid_last_error(void);  /* thread-local message of the last failure ("" if none) */
+int afid_last_error_code(void);     /* thread-local code of the last failure                 */
+const char* afid_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFID_H_ */

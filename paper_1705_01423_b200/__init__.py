@@ -1,0 +1,156 @@
+"""paper_1705_01423_b200 -- B200-native (sm_100a, fp64) projection step of AFiD (arXiv 1705.01423).
+
+Thin Python binding of the C ABI in include/afid.h (same names: afid_plan_create,
+afid_project, afid_plan_destroy, stage taps).  It only marshals arguments: every step of
+the path runs in the hand-written CUDA kernels of csrc/.  PyTorch is used by callers for
+device memory and streams; this module takes raw pointers from tensors.
+
+There is no CPU fallback: if the shared library is missing or cannot be loaded, importing
+`lib()` raises.
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libafid_b200.so")
+
+AFID_OK = 0
+ERRORS = {-1: "AFID_ERR_NULL", -2: "AFID_ERR_ALIGN", -3: "AFID_ERR_UNSUPPORTED_SIZE", -4: "AFID_ERR_GRID",
+          -5: "AFID_ERR_NOMEM", -6: "AFID_ERR_CUDA"}
+
+# every symbol include/afid.h declares
+SYMBOLS = ["afid_plan_create", "afid_project", "afid_plan_destroy", "afid_plan_workspace_bytes",
+           "afid_plan_num_launches", "afid_stage_forward", "afid_stage_solve", "afid_fft_length_supported",
+           "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version"]
+
+_lib = None
+
+
+class AfidError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{ERRORS.get(code, code)}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load libafid_b200.so (built by `python -m paper_1705_01423_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_1705_01423_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i, d = C.c_void_p, C.c_int, C.c_double
+        L.afid_plan_create.restype = vp
+        L.afid_plan_create.argtypes = [i, i, i, vp, d, d]
+        L.afid_project.restype = i
+        L.afid_project.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.afid_plan_destroy.restype = i
+        L.afid_plan_destroy.argtypes = [vp]
+        L.afid_plan_workspace_bytes.restype = C.c_size_t
+        L.afid_plan_workspace_bytes.argtypes = [vp]
+        L.afid_plan_num_launches.restype = i
+        L.afid_plan_num_launches.argtypes = [vp]
+        L.afid_stage_forward.restype = i
+        L.afid_stage_forward.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.afid_stage_solve.restype = i
+        L.afid_stage_solve.argtypes = [vp, vp, vp]
+        L.afid_fft_length_supported.restype = i
+        L.afid_fft_length_supported.argtypes = [i]
+        L.afid_max_nx.restype = i
+        L.afid_last_error.restype = C.c_char_p
+        L.afid_last_error_code.restype = i
+        L.afid_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _last_error():
+    L = lib()
+    return L.afid_last_error_code(), L.afid_last_error().decode()
+
+
+def _check(rc):
+    if rc != AFID_OK:
+        raise AfidError(rc, lib().afid_last_error().decode())
+
+
+def _dev_ptr(t, n, name):
+    """Raw device pointer of a contiguous fp64 CUDA tensor with n elements."""
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous float64 CUDA tensor")
+    if t.numel() != n:
+        raise ValueError(f"{name} has {t.numel()} elements, expected {n}")
+    return C.c_void_p(t.data_ptr())
+
+
+def fft_length_supported(n):
+    return bool(lib().afid_fft_length_supported(int(n)))
+
+
+def max_nx():
+    return int(lib().afid_max_nx())
+
+
+def version():
+    return lib().afid_version().decode()
+
+
+class Plan:
+    """afid_plan_create / afid_project / afid_plan_destroy for one grid on the current device."""
+
+    def __init__(self, nx, ny, nz, xc, Ly, Lz):
+        import numpy as np
+        xc = np.ascontiguousarray(xc, dtype=np.float64)
+        if xc.size != nx + 1:
+            raise ValueError("xc must hold nx+1 face coordinates")
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.nzh = self.nz // 2 + 1
+        self._h = lib().afid_plan_create(self.nx, self.ny, self.nz, xc.ctypes.data_as(C.c_void_p),
+                                         float(Ly), float(Lz))
+        if not self._h:
+            raise AfidError(*_last_error())
+
+    @property
+    def workspace_bytes(self):
+        return int(lib().afid_plan_workspace_bytes(self._h))
+
+    @property
+    def num_launches(self):
+        return int(lib().afid_plan_num_launches(self._h))
+
+    def _stream(self, stream):
+        import torch
+        if stream is None:
+            stream = torch.cuda.current_stream()
+        return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+    def project(self, u, v, w, p, stream=None):
+        """afid_project: u, v, w updated in place, p overwritten with phi (enqueued, no sync)."""
+        n = self.nx * self.ny * self.nz
+        _check(lib().afid_project(self._h, _dev_ptr(u, n + self.ny * self.nz, "u"), _dev_ptr(v, n, "v"),
+                                  _dev_ptr(w, n, "w"), _dev_ptr(p, n, "p"), self._stream(stream)))
+
+    def stage_forward(self, u, v, w, spec, stream=None):
+        """afid_stage_forward: spec (fp64 tensor of 2*nx*nzh*ny, complex [i][kz][ky]) <- -(D u)^/(ny nz)."""
+        n = self.nx * self.ny * self.nz
+        m = 2 * self.nx * self.nzh * self.ny
+        _check(lib().afid_stage_forward(self._h, _dev_ptr(u, n + self.ny * self.nz, "u"), _dev_ptr(v, n, "v"),
+                                        _dev_ptr(w, n, "w"), _dev_ptr(spec, m, "spec"), self._stream(stream)))
+
+    def stage_solve(self, spec, stream=None):
+        """afid_stage_solve: in-place x-solves on a [i][kz][ky] spectrum."""
+        m = 2 * self.nx * self.nzh * self.ny
+        _check(lib().afid_stage_solve(self._h, _dev_ptr(spec, m, "spec"), self._stream(stream)))
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().afid_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -1,0 +1,511 @@
+// afid_kernels.cuh -- the six kernels of one projection step (sm_100a, fp64).
+//
+//   K1 k_div_r2c     divergence (paper step 1) fused with the real-to-complex
+//                    transform along z (step 3; z is our contiguous direction)
+//   K2 k_fft_y       complex transform along y (step 5)
+//   K3 k_solve_x     tridiagonal solve along x per (ky,kz) (step 7)
+//   K4 k_ifft_y      inverse complex transform along y (step 9)
+//   K5 k_c2r_z       inverse complex-to-real transform along z (step 11) -> p = phi
+//   K6 k_correct     velocity correction u -= G phi
+//
+// The paper's pencil transposes (steps 2,4,6,8,10,12) become the tile gathers of K2..K5:
+// every kernel writes its output contiguously and the NEXT kernel gathers >=128-byte
+// segments (measured on B200: segmented reads of >=256 B run at copy speed, segmented
+// writes do not).  Work-array layouts (complex doubles; nzh = nz/2+1, NJT = ny/8):
+//   B  [i][jt][kz][8]     written by K1   (8 = j within the tile jt)
+//   C  [i][kz][ky]        written by K2
+//   T  [kz][kyt][i][8]    written by K3   (8 = ky within the tile kyt)
+//   D  [i][kz][j]         written by K4
+#pragma once
+#include "fft_device.cuh"
+
+namespace afid {
+
+struct DevParams {
+    int nx, ny, nz, nzh;
+    double rdy, rdz;            // 1/dy, 1/dz
+    double spec_scale;          // -1/(ny*nz): folded into K1's post-processing
+    const double* rdx;          // [nx]   1/dx_i
+    const double* rdc;          // [nx+1] 1/dc_i (faces 1..nx-1; 0 at the walls)
+    const double* dxw;          // [nx]   dx_i (weights of the mean)
+    const double* ca;           // [nx]   a_i = 1/(dx_i dc_i),   a_0 = 0
+    const double* cc;           // [nx]   c_i = 1/(dx_i dc_{i+1}), c_{nx-1} = 0
+    const double* lamy;         // [ny]   modified wavenumbers in y
+    const double* lamz;         // [nzh]  modified wavenumbers in z
+    const cplx* tw_y;           // [ny]    exp(-2 pi i k/ny)
+    const cplx* tw_zh;          // [nz/2]  exp(-2 pi i k/(nz/2))
+    const cplx* tw_z;           // [nz/2+1] exp(-2 pi i k/nz)
+    double inv_vol;             // 1/sum dx_i
+};
+
+__device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
+
+// ------------------------------------------------------------------------------------------
+// K1: divergence + r2c along z.  CTA = (i, group of NL consecutive j); NL*TPL threads.
+// The real line d(i,j,0..nz-1) is transformed as the complex line z(m) = d(2m) + i d(2m+1)
+// of length Nh = nz/2, then split:  X(k) = 1/2 [ (Z(k)+conj Z(Nh-k)) - i w_nz^k (Z(k)-conj Z(Nh-k)) ].
+// Output: B[i][jt][kz][jl] = spec_scale * X(kz), kz = 0..Nh.
+// ------------------------------------------------------------------------------------------
+template <class PL, int NL>
+__global__ void __launch_bounds__(NL* PL::TPL) k_div_r2c(DevParams P, const double* __restrict__ u,
+                                                         const double* __restrict__ v, const double* __restrict__ w,
+                                                         cplx* __restrict__ B)
+{
+    constexpr int Nh = PL::N, TPL = PL::TPL, LS = PL::LS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* sm = reinterpret_cast<cplx*>(smem_raw);
+    const int ngrp = P.ny / NL;
+    const int i = blockIdx.x / ngrp, jg = blockIdx.x % ngrp;
+    const int ln = threadIdx.x / TPL, tl = threadIdx.x % TPL;
+    const int j = jg * NL + ln;
+    const int jp = (j + 1 == P.ny) ? 0 : j + 1;
+    const size_t plane = (size_t)P.ny * P.nz;
+    const double* u0 = u + (size_t)i * plane + (size_t)j * P.nz;
+    const double* u1 = u0 + plane;
+    const double* v0 = v + (size_t)i * plane + (size_t)j * P.nz;
+    const double* v1 = v + (size_t)i * plane + (size_t)jp * P.nz;
+    const double* w0 = w + (size_t)i * plane + (size_t)j * P.nz;
+    const double rdx = __ldg(&P.rdx[i]), rdy = P.rdy, rdz = P.rdz;
+    cplx* line = sm + ln * LS;
+
+    // divergence of the two cells 2e, 2e+1 (P:L87 stencil)
+    auto ld_div = [&](int e) -> cplx {
+        const double2 a1 = ldg2(u1 + 2 * e), a0 = ldg2(u0 + 2 * e);
+        const double2 b1 = ldg2(v1 + 2 * e), b0 = ldg2(v0 + 2 * e);
+        const double2 c0 = ldg2(w0 + 2 * e);
+        const double cn = __ldg(w0 + ((e == Nh - 1) ? 0 : 2 * e + 2));
+        cplx d;
+        d.x = (a1.x - a0.x) * rdx + (b1.x - b0.x) * rdy + (c0.y - c0.x) * rdz;
+        d.y = (a1.y - a0.y) * rdx + (b1.y - b0.y) * rdy + (cn - c0.y) * rdz;
+        return d;
+    };
+    {
+        typedef FftPass<PL, 0> P0;
+        typename P0::Regs rg;
+        P0::load(rg, tl, ld_div);
+        P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { line[PL::pad(e)] = val; });
+    }
+    fft_tail_passes<PL, 1, true>(line, tl, true, P.tw_zh, [](int, cplx) {});
+
+    // split into the spectrum of the real line; thread -> (k, jl) with jl fastest
+    const int jl0 = (jg * NL) % 8;         // position of this CTA's first line inside the tile
+    cplx* out = B + ((size_t)i * (P.ny / 8) + (size_t)(jg * NL / 8)) * (size_t)P.nzh * 8;
+    const double hs = 0.5 * P.spec_scale;
+    for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NL * TPL) {
+        const int k = idx / NL, l = idx % NL;
+        const cplx* zl = sm + l * LS;
+        const cplx zk = zl[PL::pad(k)];
+        const cplx zm = zl[PL::pad(k == 0 ? 0 : Nh - k)];
+        // E = Z(k) + conj Z(Nh-k);  O = Z(k) - conj Z(Nh-k)
+        const cplx E = mk(zk.x + zm.x, zk.y - zm.y), O = mk(zk.x - zm.x, zk.y + zm.y);
+        const cplx wk = __ldg(&P.tw_z[k]); // exp(-2 pi i k / nz)
+        // -i w O
+        const cplx wo = cmul(wk, O);
+        const cplx t = mk(wo.y, -wo.x);
+        const cplx xk = mk(hs * (E.x + t.x), hs * (E.y + t.y));
+        // X(Nh-k) = 1/2 [ conj(E) ... ]: by symmetry X(Nh-k) = 1/2 conj( E + i w O ) ... derived below
+        // Z(Nh-k) + conj Z(k) = conj(E);  Z(Nh-k) - conj Z(k) = -conj(O);  w^(Nh-k) = -conj(w^k)
+        // X(Nh-k) = 1/2 [ conj(E) - i (-conj w)(-conj O) ] = 1/2 [ conj(E) - i conj(w O) ] = 1/2 conj( E + i w O )
+        const cplx xm = mk(hs * (E.x - t.x), -hs * (E.y - t.y));
+        out[(size_t)k * 8 + jl0 + l] = xk;
+        if (k != Nh - k) out[(size_t)(Nh - k) * 8 + jl0 + l] = xm;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// K2: forward complex FFT along y.  CTA = (i, NL consecutive kz); reads B (segments of
+// NL*128 bytes), writes C[i][kz][ky] contiguously.
+// ------------------------------------------------------------------------------------------
+template <class PL> constexpr int tpl8() { return (PL::TPL + 7) / 8 * 8; }
+
+template <class PL, int NL>
+__global__ void __launch_bounds__(NL* tpl8<PL>()) k_fft_y(DevParams P, const cplx* __restrict__ B, cplx* __restrict__ C)
+{
+    constexpr int TPL = PL::TPL, LS = PL::LS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* sm = reinterpret_cast<cplx*>(smem_raw);
+    const int ngrp = (P.nzh + NL - 1) / NL;
+    const int i = blockIdx.x / ngrp, kg = blockIdx.x % ngrp;
+    // interleave the NL lines at 8-thread granularity so that a warp's loads cover
+    // NL*128 contiguous bytes of B
+    const int ln = (threadIdx.x >> 3) % NL;
+    const int tl = (threadIdx.x & 7) | ((threadIdx.x / (8 * NL)) << 3);
+    const int kz = kg * NL + ln;
+    const bool active = (kz < P.nzh) && (tl < TPL);
+    const cplx* src = B + (size_t)i * (P.ny / 8) * (size_t)P.nzh * 8 + (size_t)kz * 8;
+    const size_t tile_stride = (size_t)P.nzh * 8;
+    cplx* dst = C + ((size_t)i * P.nzh + kz) * (size_t)P.ny;
+    cplx* line = sm + ln * LS;
+    auto ld_b = [&](int e) -> cplx { return __ldg(&src[(size_t)(e >> 3) * tile_stride + (e & 7)]); };
+    auto st_c = [&](int e, cplx val) { dst[e] = val; };
+    typedef FftPass<PL, 0> P0;
+    if constexpr (PL::NPASS == 1) {
+        if (active) {
+            typename P0::Regs rg;
+            P0::load(rg, tl, ld_b);
+            P0::compute_store(rg, tl, P.tw_y, st_c);
+        }
+    } else {
+        if (active) {
+            typename P0::Regs rg;
+            P0::load(rg, tl, ld_b);
+            P0::compute_store(rg, tl, P.tw_y, [&](int e, cplx val) { line[PL::pad(e)] = val; });
+        }
+        fft_tail_passes<PL, 1, false>(line, tl, active, P.tw_y, st_c);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// K4: inverse complex FFT along y (unnormalised; the 1/(ny nz) is in spec_scale).
+// CTA = (NL consecutive i, kz); reads T[kz][kyt][i][8] (segments of NL*128 bytes), writes
+// D[i][kz][j] contiguously.  Inverse = forward with re/im swapped on load and store.
+// ------------------------------------------------------------------------------------------
+template <class PL, int NL>
+__global__ void __launch_bounds__(NL* tpl8<PL>()) k_ifft_y(DevParams P, const cplx* __restrict__ T, cplx* __restrict__ D)
+{
+    constexpr int TPL = PL::TPL, LS = PL::LS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* sm = reinterpret_cast<cplx*>(smem_raw);
+    const int ngrp = (P.nx + NL - 1) / NL;
+    const int kz = blockIdx.x / ngrp, ig = blockIdx.x % ngrp;
+    const int ln = (threadIdx.x >> 3) % NL;
+    const int tl = (threadIdx.x & 7) | ((threadIdx.x / (8 * NL)) << 3);
+    const int i = ig * NL + ln;
+    const bool active = (i < P.nx) && (tl < TPL);
+    const size_t tile_stride = (size_t)P.nx * 8;
+    const cplx* src = T + (size_t)kz * (P.ny / 8) * tile_stride + (size_t)i * 8;
+    cplx* dst = D + ((size_t)i * P.nzh + kz) * (size_t)P.ny;
+    cplx* line = sm + ln * LS;
+    auto ld_t = [&](int e) -> cplx { return cswap(__ldg(&src[(size_t)(e >> 3) * tile_stride + (e & 7)])); };
+    auto st_d = [&](int e, cplx val) { dst[e] = cswap(val); };
+    typedef FftPass<PL, 0> P0;
+    if constexpr (PL::NPASS == 1) {
+        if (active) {
+            typename P0::Regs rg;
+            P0::load(rg, tl, ld_t);
+            P0::compute_store(rg, tl, P.tw_y, st_d);
+        }
+    } else {
+        if (active) {
+            typename P0::Regs rg;
+            P0::load(rg, tl, ld_t);
+            P0::compute_store(rg, tl, P.tw_y, [&](int e, cplx val) { line[PL::pad(e)] = val; });
+        }
+        fft_tail_passes<PL, 1, false>(line, tl, active, P.tw_y, st_d);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// K5: inverse c2r along z -> p.  CTA = (i, tile of 8 consecutive j); 8*TPL threads.
+// Gathers D[i][kz][8 j] (128-byte segments), forms Z'(k) = (X(k)+conj X(Nh-k)) + i conj(w^k)(X(k)-conj X(Nh-k)),
+// inverse complex FFT of length Nh gives z(m) = phi(2m) + i phi(2m+1).
+// ------------------------------------------------------------------------------------------
+template <class PL>
+__global__ void __launch_bounds__(8 * PL::TPL) k_c2r_z(DevParams P, const cplx* __restrict__ D, double* __restrict__ p)
+{
+    constexpr int Nh = PL::N, TPL = PL::TPL, LS = PL::LS, NL = 8;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* sm = reinterpret_cast<cplx*>(smem_raw);
+    const int njt = P.ny / 8;
+    const int i = blockIdx.x / njt, jt = blockIdx.x % njt;
+    const cplx* src = D + (size_t)i * P.nzh * (size_t)P.ny + (size_t)jt * 8;
+    for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NL * TPL) {
+        const int k = idx >> 3, l = idx & 7;
+        const int km = Nh - k;
+        const cplx xk = __ldg(&src[(size_t)k * P.ny + l]);
+        const cplx xm = __ldg(&src[(size_t)km * P.ny + l]);
+        const cplx wk = __ldg(&P.tw_z[k]);
+        // E = X(k) + conj X(Nh-k), O = X(k) - conj X(Nh-k)
+        const cplx E = mk(xk.x + xm.x, xk.y - xm.y), O = mk(xk.x - xm.x, xk.y + xm.y);
+        // i conj(w) O
+        const cplx wo = mk(fma(wk.y, O.y, wk.x * O.x), fma(-wk.y, O.x, wk.x * O.y)); // conj(w) * O
+        const cplx t = mk(-wo.y, wo.x);
+        cplx* zl = sm + l * LS;
+        // stored re/im-swapped: the inverse transform runs as a forward one on swapped data
+        zl[PL::pad(k)] = mk(E.y + t.y, E.x + t.x);
+        // Z'(Nh-k) = conj(E) + i conj(w^(Nh-k)) (-conj O) = conj(E) + i w^k ... = conj( E - i conj(w) O )
+        if (k != 0 && k != km) zl[PL::pad(km)] = mk(-(E.y - t.y), E.x - t.x);
+    }
+    __syncthreads();
+    const int ln = threadIdx.x / TPL, tl = threadIdx.x % TPL;
+    cplx* line = sm + ln * LS;
+    double* dst = p + ((size_t)i * P.ny + (size_t)jt * 8 + ln) * (size_t)P.nz;
+    auto st_p = [&](int e, cplx val) { reinterpret_cast<double2*>(dst)[e] = cswap(val); };
+    typedef FftPass<PL, 0> P0;
+    {
+        typename P0::Regs rg;
+        P0::load(rg, tl, [&](int e) { return line[PL::pad(e)]; });
+        if constexpr (PL::NPASS == 1) {
+            P0::compute_store(rg, tl, P.tw_zh, st_p);
+        } else {
+            __syncthreads();
+            P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { line[PL::pad(e)] = val; });
+        }
+    }
+    if constexpr (PL::NPASS > 1) fft_tail_passes<PL, 1, false>(line, tl, true, P.tw_zh, st_p);
+}
+
+// ------------------------------------------------------------------------------------------
+// K6: correction.  One thread per pair of cells (k, k+1).
+//   u[i] -= (phi[i]-phi[i-1])/dc_i (i >= 1; wall planes untouched), v -= d_y phi/dy, w -= d_z phi/dz.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_correct(DevParams P, const double* __restrict__ p, double* __restrict__ u,
+                                                 double* __restrict__ v, double* __restrict__ w)
+{
+    const int nzh2 = P.nz / 2;
+    const size_t npair = (size_t)P.nx * P.ny * nzh2;
+    const size_t plane = (size_t)P.ny * P.nz;
+    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < npair; t += (size_t)gridDim.x * blockDim.x) {
+        const int kp = (int)(t % nzh2);
+        const size_t ij = t / nzh2;
+        const int j = (int)(ij % P.ny), i = (int)(ij / P.ny);
+        const size_t o = ij * P.nz + 2 * (size_t)kp;
+        const double2 ph = ldg2(p + o);
+        const size_t ojm = (j == 0) ? o + (size_t)(P.ny - 1) * P.nz : o - P.nz;
+        const double2 pj = ldg2(p + ojm);
+        const double pk = __ldg(p + (kp == 0 ? ij * P.nz + P.nz - 1 : o - 1));
+        double2 vv = *reinterpret_cast<double2*>(v + o), ww = *reinterpret_cast<double2*>(w + o);
+        vv.x -= (ph.x - pj.x) * P.rdy;
+        vv.y -= (ph.y - pj.y) * P.rdy;
+        ww.x -= (ph.x - pk) * P.rdz;
+        ww.y -= (ph.y - ph.x) * P.rdz;
+        *reinterpret_cast<double2*>(v + o) = vv;
+        *reinterpret_cast<double2*>(w + o) = ww;
+        if (i >= 1) {
+            const double2 pi = ldg2(p + o - plane);
+            const double r = __ldg(&P.rdc[i]);
+            double2 uu = *reinterpret_cast<double2*>(u + o);
+            uu.x -= (ph.x - pi.x) * r;
+            uu.y -= (ph.y - pi.y) * r;
+            *reinterpret_cast<double2*>(u + o) = uu;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// K3: tridiagonal solves along x (paper step 7).  For every mode (ky,kz), lam = lamy+lamz:
+//     -a_i x_{i-1} + (a_i + c_i + lam) x_i - c_i x_{i+1} = f_i ,   f = -dhat/(ny nz)  (from K1)
+// (the paper's system a x_{i-1} - (a+c+lam) x_i + c x_{i+1} = dhat with the sign flipped so
+// that the matrix is an M-matrix).  CTA = 8 consecutive ky of one kz; the 8 whole columns
+// (nx x 8 complex) sit in shared memory; thread (s, q) owns the chunk of M rows q of system s.
+//
+// Parallel-in-x algorithm, every quantity a sum/product of non-negative numbers (no
+// cancellation at small lam):
+//   chunk q = rows [qM, qM+M); its last row is an INTERFACE unknown E_q, the others are interior.
+//   interior row elimination toward a boundary carries  x_i = y_i + g_i x_next + h_i E_far
+//   with g + h + t = 1 and   nh = a h', nt = lam + a t', pi = c + nh + nt,
+//                            h = nh/pi, t = nt/pi, g = c/pi, y = (f + a y')/pi      (downward; upward: a<->c)
+//   -> reduced system in E of the same form: -A_q E_{q-1} + (A_q + C_q + L_q) E_q - C_q E_{q+1} = F_q
+//      A_q = a h, C_q = c h^, L_q = lam + a t + c t^, F_q = f + a y + c y^
+//   -> solved by cancellation-free parallel cyclic reduction across the P threads of a system
+//      (L' = L + alpha L_- + gamma L_+ stays a sum of non-negatives)
+//   -> interior rows by back substitution x_i = y_i + g_i x_{i+1} + h_i E_{q-1}.
+// Mode (0,0) (lam = 0, singular; R7): last row pinned to 0, then the dx-weighted
+// mean is subtracted.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double fast_rcp(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    return r;
+}
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+template <int M>
+__global__ void __launch_bounds__(M == 4 ? 128 : (M == 16 ? 512 : 384)) k_solve_x(DevParams P, const cplx* __restrict__ C, cplx* __restrict__ T)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int nx = P.nx, PCH = blockDim.x >> 3;
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw);            // [nx][8]
+    double* red = reinterpret_cast<double*>(tile + (size_t)nx * 8); // 2 buffers x 5 arrays x [PCH][8]
+    const int nkt = P.ny / 8;
+    const int kz = blockIdx.x / nkt, kyt = blockIdx.x % nkt;
+    const int s = threadIdx.x & 7, q = threadIdx.x >> 3;
+    const int slot = q * 8 + s, NS = PCH * 8;
+
+    {   // gather the 8 columns: 128-byte segments of C[i][kz][ky]
+        const cplx* src = C + (size_t)kz * P.ny + (size_t)kyt * 8 + s;
+        const size_t rs = (size_t)P.nzh * P.ny;
+        for (int i = q; i < nx; i += PCH) cp_async16(&tile[i * 8 + s], src + (size_t)i * rs);
+        cp_async_wait_all();
+        __syncthreads();
+    }
+    const double lam = __ldg(&P.lamy[kyt * 8 + s]) + __ldg(&P.lamz[kz]);
+    const bool cta_singular = (blockIdx.x == 0);
+    const int i0 = q * M;
+    const int i1 = min(i0 + M, nx) - 1; // interface row of this chunk
+    double* bA = red;
+    double* bC = red + NS;
+    double* bL = red + 2 * NS;
+    double* bFr = red + 3 * NS;
+    double* bFi = red + 4 * NS;
+    double* nA = red + 5 * NS;
+    double* nC = nA + NS;
+    double* nL = nA + 2 * NS;
+    double* nFr = nA + 3 * NS;
+    double* nFi = nA + 4 * NS;
+
+    // upward elimination of the interior (read only): relation of the first interior row
+    {
+        double h = 1.0, t = 0.0, yr = 0.0, yi = 0.0;
+#pragma unroll
+        for (int r = M - 2; r >= 0; --r) {
+            const int i = i0 + r;
+            if (i < i1) {
+                const double a = __ldg(&P.ca[i]), c = __ldg(&P.cc[i]);
+                const double nh = c * h, nt = fma(c, t, lam);
+                const double rr = fast_rcp(a + (nh + nt));
+                const cplx f = tile[i * 8 + s];
+                h = nh * rr;
+                t = nt * rr;
+                yr = fma(c, yr, f.x) * rr;
+                yi = fma(c, yi, f.y) * rr;
+            }
+        }
+        if (q > 0) { // contribution to the interface row above (reduced row q-1); staged in the "next" buffer
+            const double cb = __ldg(&P.cc[i0 - 1]);
+            nC[slot - 8] = cb * h;
+            nL[slot - 8] = cb * t;
+            nFr[slot - 8] = cb * yr;
+            nFi[slot - 8] = cb * yi;
+        }
+    }
+    // downward elimination of the interior (in place: tile <- y), keeping g, h in registers
+    double G[M - 1 > 0 ? M - 1 : 1], H[M - 1 > 0 ? M - 1 : 1];
+    double rA, rC, rL, rFr, rFi;
+    {
+        double h = 1.0, t = 0.0, yr = 0.0, yi = 0.0;
+#pragma unroll
+        for (int r = 0; r < M - 1; ++r) {
+            const int i = i0 + r;
+            if (i < i1) {
+                const double a = __ldg(&P.ca[i]), c = __ldg(&P.cc[i]);
+                const double nh = a * h, nt = fma(a, t, lam);
+                const double rr = fast_rcp(c + (nh + nt));
+                const cplx f = tile[i * 8 + s];
+                h = nh * rr;
+                t = nt * rr;
+                yr = fma(a, yr, f.x) * rr;
+                yi = fma(a, yi, f.y) * rr;
+                tile[i * 8 + s] = mk(yr, yi);
+                G[r] = c * rr;
+                H[r] = h;
+            }
+        }
+        const double ab = __ldg(&P.ca[i1]);
+        const cplx f = tile[i1 * 8 + s];
+        rA = ab * h;
+        rL = fma(ab, t, lam);
+        rFr = fma(ab, yr, f.x);
+        rFi = fma(ab, yi, f.y);
+    }
+    __syncthreads();
+    if (q < PCH - 1) {
+        rC = nC[slot];
+        rL += nL[slot];
+        rFr += nFr[slot];
+        rFi += nFi[slot];
+    } else {
+        rC = 0.0;
+    }
+    if (cta_singular && s == 0 && q == PCH - 1) { // pin the last unknown of the mean mode
+        rA = 0.0; rC = 0.0; rL = 1.0; rFr = 0.0; rFi = 0.0;
+    }
+    // cancellation-free PCR over the PCH interface unknowns of each system
+    for (int d = 1; d < PCH; d <<= 1) {
+        bA[slot] = rA; bC[slot] = rC; bL[slot] = rL; bFr[slot] = rFr; bFi[slot] = rFi;
+        __syncthreads();
+        double A2 = 0.0, C2 = 0.0;
+        if (q - d >= 0) {
+            const int m = slot - 8 * d;
+            const double Am = bA[m], Lm = bL[m];
+            const double al = rA * fast_rcp(Am + bC[m] + Lm);
+            A2 = al * Am;
+            rL = fma(al, Lm, rL);
+            rFr = fma(al, bFr[m], rFr);
+            rFi = fma(al, bFi[m], rFi);
+        }
+        if (q + d < PCH) {
+            const int m = slot + 8 * d;
+            const double Cp = bC[m], Lp = bL[m];
+            const double ga = rC * fast_rcp(bA[m] + Cp + Lp);
+            C2 = ga * Cp;
+            rL = fma(ga, Lp, rL);
+            rFr = fma(ga, bFr[m], rFr);
+            rFi = fma(ga, bFi[m], rFi);
+        }
+        rA = A2;
+        rC = C2;
+        // swap buffers
+        double* tp;
+        tp = bA; bA = nA; nA = tp;
+        tp = bC; bC = nC; nC = tp;
+        tp = bL; bL = nL; nL = tp;
+        tp = bFr; bFr = nFr; nFr = tp;
+        tp = bFi; bFi = nFi; nFi = tp;
+    }
+    {
+        const double rr = fast_rcp(rA + rC + rL);
+        const double er = rFr * rr, ei = rFi * rr;
+        bFr[slot] = er;
+        bFi[slot] = ei;
+        __syncthreads();
+        const double elr = (q > 0) ? bFr[slot - 8] : 0.0, eli = (q > 0) ? bFi[slot - 8] : 0.0;
+        double xr = er, xi = ei;
+        tile[i1 * 8 + s] = mk(xr, xi);
+#pragma unroll
+        for (int r = M - 2; r >= 0; --r) {
+            const int i = i0 + r;
+            if (i < i1) {
+                const cplx y = tile[i * 8 + s];
+                xr = fma(G[r], xr, fma(H[r], elr, y.x));
+                xi = fma(G[r], xi, fma(H[r], eli, y.y));
+                tile[i * 8 + s] = mk(xr, xi);
+            }
+        }
+    }
+    __syncthreads();
+    if (cta_singular) { // zero dx-weighted mean for mode (0,0) = system s = 0 of this CTA
+        if (s == 0) {
+            double sr = 0.0, si = 0.0;
+            for (int i = i0; i <= i1; ++i) {
+                const double wgt = __ldg(&P.dxw[i]);
+                const cplx x = tile[i * 8];
+                sr = fma(x.x, wgt, sr);
+                si = fma(x.y, wgt, si);
+            }
+            nFr[q] = sr;
+            nFi[q] = si;
+        }
+        __syncthreads();
+        if (s == 0) {
+            double sr = 0.0, si = 0.0;
+            for (int qq = 0; qq < PCH; ++qq) { sr += nFr[qq]; si += nFi[qq]; }
+            sr *= P.inv_vol;
+            si *= P.inv_vol;
+            for (int i = i0; i <= i1; ++i) {
+                cplx x = tile[i * 8];
+                x.x -= sr;
+                x.y -= si;
+                tile[i * 8] = x;
+            }
+        }
+        __syncthreads();
+    }
+    {   // contiguous store of the tile: T[kz][kyt][i][8]
+        cplx* dst = T + ((size_t)kz * nkt + kyt) * (size_t)nx * 8;
+        for (int e = threadIdx.x; e < nx * 8; e += blockDim.x) dst[e] = tile[e];
+    }
+}
+
+} // namespace afid

@@ -1,0 +1,355 @@
+// afid_plan.cu -- host side of the C ABI in include/afid.h: plan construction (metrics,
+// tridiagonal coefficients, modified wavenumbers, twiddle tables), validation, and the
+// launch sequence of one projection.  No CPU fallback and no library FFT: an unsupported
+// size is an error.
+#include "../../include/afid.h"
+#include "afid_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace afid;
+
+namespace {
+
+thread_local std::string g_err;
+thread_local int g_err_code = 0;
+
+int fail(int code, const std::string& msg)
+{
+    g_err = msg;
+    g_err_code = code;
+    return code;
+}
+
+// ---- FFT length table: complex length -> radix plan and threads per line ------------------
+//      X(N, R0, R1, R2, R3, TPL)
+#define AFID_FFT_SIZES(X)       \
+    X(8, 8, 1, 1, 1, 1)         \
+    X(16, 16, 1, 1, 1, 1)       \
+    X(24, 8, 3, 1, 1, 3)        \
+    X(32, 8, 4, 1, 1, 4)        \
+    X(48, 16, 3, 1, 1, 4)       \
+    X(64, 8, 8, 1, 1, 8)        \
+    X(96, 16, 6, 1, 1, 8)       \
+    X(128, 16, 8, 1, 1, 8)      \
+    X(192, 16, 12, 1, 1, 16)    \
+    X(256, 16, 16, 1, 1, 16)    \
+    X(384, 8, 8, 6, 1, 48)      \
+    X(512, 8, 8, 8, 1, 64)      \
+    X(768, 16, 16, 3, 1, 48)    \
+    X(1024, 16, 8, 8, 1, 64)    \
+    X(1536, 16, 16, 6, 1, 96)   \
+    X(2048, 16, 16, 8, 1, 128)  \
+    X(3072, 16, 16, 12, 1, 192) \
+    X(4096, 16, 16, 16, 1, 256)
+
+constexpr int K1_NL = 4; // lines per CTA in K1 (two CTAs fill one 128-byte row of B)
+constexpr int KY_NL = 2; // lines per CTA in K2 / K4 (256-byte gather segments)
+constexpr int MAX_ZH = 1024; // largest nz/2 for which K5's 8-line tile fits shared memory
+
+struct LaunchCfg {
+    const void* fn;
+    int threads;
+    size_t smem;
+};
+
+template <class PL> LaunchCfg cfg_k1()
+{
+    return {(const void*)k_div_r2c<PL, K1_NL>, K1_NL * PL::TPL, (size_t)K1_NL * PL::LS * sizeof(cplx)};
+}
+template <class PL> LaunchCfg cfg_k2()
+{
+    return {(const void*)k_fft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx)};
+}
+template <class PL> LaunchCfg cfg_k4()
+{
+    return {(const void*)k_ifft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx)};
+}
+template <class PL> LaunchCfg cfg_k5()
+{
+    return {(const void*)k_c2r_z<PL>, 8 * PL::TPL, (size_t)8 * PL::LS * sizeof(cplx)};
+}
+
+bool lookup_fft(int n, LaunchCfg* k1, LaunchCfg* k2, LaunchCfg* k4, LaunchCfg* k5)
+{
+    switch (n) {
+#define X(N, R0, R1, R2, R3, TPL)                   \
+    case N: {                                       \
+        typedef FftPlan<R0, R1, R2, R3, TPL> PL;    \
+        if (k1) *k1 = cfg_k1<PL>();                 \
+        if (k2) *k2 = cfg_k2<PL>();                 \
+        if (k4) *k4 = cfg_k4<PL>();                 \
+        if (k5) *k5 = cfg_k5<PL>();                 \
+        return true;                                \
+    }
+        AFID_FFT_SIZES(X)
+#undef X
+    default:
+        return false;
+    }
+}
+
+constexpr int MAX_NX = 1536;
+
+} // namespace
+
+struct afid_plan {
+    int nx, ny, nz, nzh;
+    DevParams dp;
+    void* tables;      // one device allocation holding all tables
+    size_t tables_bytes;
+    cplx* ws[2];       // work arrays, nx*nzh*ny complex each
+    size_t ws_bytes;
+    LaunchCfg k1, k2, k4, k5, k3;
+    int k3_threads;
+    int n_sm;
+};
+
+extern "C" {
+
+const char* afid_version(void) { return "afid-project-b200 0.1 (sm_100a, fp64)"; }
+const char* afid_last_error(void) { return g_err.c_str(); }
+int afid_last_error_code(void) { return g_err_code; }
+int afid_max_nx(void) { return MAX_NX; }
+int afid_fft_length_supported(int n) { return lookup_fft(n, nullptr, nullptr, nullptr, nullptr) ? 1 : 0; }
+
+static int set_smem_attr(const LaunchCfg& c)
+{
+    if (c.smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(c.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+        if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+    }
+    return AFID_OK;
+}
+
+afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly, double Lz)
+{
+    g_err.clear();
+    g_err_code = 0;
+    if (!xc) { fail(AFID_ERR_NULL, "xc is NULL"); return nullptr; }
+    if (nx < 2 || nx > MAX_NX) { fail(AFID_ERR_UNSUPPORTED_SIZE, "nx must be in [2, afid_max_nx()]"); return nullptr; }
+    if (ny < 8 || nz < 16 || (nz & 1)) { fail(AFID_ERR_UNSUPPORTED_SIZE, "ny >= 8 and even nz >= 16 required"); return nullptr; }
+    if (!(Ly > 0.0) || !(Lz > 0.0) || !std::isfinite(Ly) || !std::isfinite(Lz)) { fail(AFID_ERR_GRID, "Ly, Lz must be finite and > 0"); return nullptr; }
+    for (int i = 0; i <= nx; ++i)
+        if (!std::isfinite(xc[i]) || (i > 0 && !(xc[i] > xc[i - 1]))) { fail(AFID_ERR_GRID, "xc must be finite and strictly increasing"); return nullptr; }
+    const int nh = nz / 2;
+    afid_plan* pl = new (std::nothrow) afid_plan();
+    if (!pl) { fail(AFID_ERR_NOMEM, "host allocation failed"); return nullptr; }
+    std::memset(pl, 0, sizeof(*pl));
+    if (!lookup_fft(ny, nullptr, &pl->k2, &pl->k4, nullptr)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "ny is not a supported FFT length"); return nullptr; }
+    if (nh > MAX_ZH || !lookup_fft(nh, &pl->k1, nullptr, nullptr, &pl->k5)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "nz/2 is not a supported FFT length"); return nullptr; }
+    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
+
+    // ---- K3 configuration
+    int M, pch;
+    if (nx < 64) { M = 4; pl->k3.fn = (const void*)k_solve_x<4>; }
+    else if (nx <= 1024) { M = 16; pl->k3.fn = (const void*)k_solve_x<16>; }
+    else { M = 32; pl->k3.fn = (const void*)k_solve_x<32>; }
+    pch = (nx + M - 1) / M;
+    pl->k3.threads = 8 * pch;
+    pl->k3.smem = (size_t)nx * 8 * sizeof(cplx) + (size_t)10 * pch * 8 * sizeof(double);
+
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        delete pl; fail(AFID_ERR_CUDA, "no CUDA device"); return nullptr;
+    }
+    if (prop.major != 10) { delete pl; fail(AFID_ERR_CUDA, "this library is built for sm_100a (B200) only"); return nullptr; }
+    pl->n_sm = prop.multiProcessorCount;
+    for (const LaunchCfg* c : {&pl->k1, &pl->k2, &pl->k3, &pl->k4, &pl->k5}) {
+        if (c->smem > prop.sharedMemPerBlockOptin) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "tile does not fit shared memory"); return nullptr; }
+        if (set_smem_attr(*c) != AFID_OK) { delete pl; return nullptr; }
+    }
+
+    // ---- host tables (long double, rounded once to fp64)
+    typedef long double ld;
+    std::vector<double> dx(nx), dc(nx + 1, 0.0), rdx(nx), rdc(nx + 1, 0.0), ca(nx, 0.0), cc(nx, 0.0), lamy(ny), lamz(nh + 1);
+    // metrics: one fp64 subtraction of the inputs each (R1/R4)
+    for (int i = 0; i < nx; ++i) dx[i] = xc[i + 1] - xc[i];
+    for (int i = 1; i < nx; ++i) dc[i] = (xc[i + 1] - xc[i - 1]) / 2.0;
+    ld vol = 0.0L;
+    for (int i = 0; i < nx; ++i) {
+        rdx[i] = (double)(1.0L / (ld)dx[i]);
+        vol += (ld)dx[i];
+        if (i >= 1) { rdc[i] = (double)(1.0L / (ld)dc[i]); ca[i] = (double)(1.0L / ((ld)dx[i] * (ld)dc[i])); }
+        if (i <= nx - 2) cc[i] = (double)(1.0L / ((ld)dx[i] * (ld)dc[i + 1]));
+    }
+    const ld pi = acosl(-1.0L);
+    const double dy = Ly / ny, dz = Lz / nz;
+    // modified wavenumbers 2(1-cos(2 pi k/n))/Delta^2 = 4 sin^2(pi k/n)/Delta^2
+    for (int k = 0; k < ny; ++k) { ld s = sinl(pi * (ld)k / (ld)ny); lamy[k] = (double)(4.0L * s * s / ((ld)dy * (ld)dy)); }
+    for (int k = 0; k <= nh; ++k) { ld s = sinl(pi * (ld)k / (ld)nz); lamz[k] = (double)(4.0L * s * s / ((ld)dz * (ld)dz)); }
+    std::vector<double> twy(2 * (size_t)ny), twzh(2 * (size_t)nh), twz(2 * (size_t)(nh + 1));
+    auto fill_tw = [&](std::vector<double>& t, int count, int n) {
+        for (int k = 0; k < count; ++k) {
+            // reduce to the first octant for accuracy
+            const ld ang = 2.0L * pi * (ld)k / (ld)n;
+            t[2 * k] = (double)cosl(ang);
+            t[2 * k + 1] = (double)(-sinl(ang));
+        }
+    };
+    fill_tw(twy, ny, ny);
+    fill_tw(twzh, nh, nh);
+    fill_tw(twz, nh + 1, nz);
+
+    // ---- one device allocation for all tables (each sub-table 256-byte aligned)
+    struct Item { const void* src; size_t bytes; size_t off; };
+    std::vector<Item> items = {
+        {rdx.data(), rdx.size() * 8, 0}, {rdc.data(), rdc.size() * 8, 0}, {dx.data(), dx.size() * 8, 0},
+        {ca.data(), ca.size() * 8, 0},   {cc.data(), cc.size() * 8, 0},   {lamy.data(), lamy.size() * 8, 0},
+        {lamz.data(), lamz.size() * 8, 0}, {twy.data(), twy.size() * 8, 0}, {twzh.data(), twzh.size() * 8, 0},
+        {twz.data(), twz.size() * 8, 0}};
+    size_t off = 0;
+    for (auto& it : items) { it.off = off; off += (it.bytes + 255) / 256 * 256; }
+    pl->tables_bytes = off;
+    if (cudaMalloc(&pl->tables, off) != cudaSuccess) { cudaGetLastError(); delete pl; fail(AFID_ERR_NOMEM, "cudaMalloc(tables) failed"); return nullptr; }
+    for (auto& it : items)
+        if (cudaMemcpy((char*)pl->tables + it.off, it.src, it.bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaFree(pl->tables); delete pl; fail(AFID_ERR_CUDA, "cudaMemcpy(tables) failed"); return nullptr;
+        }
+    pl->ws_bytes = (size_t)nx * pl->nzh * ny * sizeof(cplx);
+    for (int b = 0; b < 2; ++b)
+        if (cudaMalloc((void**)&pl->ws[b], pl->ws_bytes) != cudaSuccess) {
+            cudaGetLastError();
+            if (b == 1) cudaFree(pl->ws[0]);
+            cudaFree(pl->tables); delete pl; fail(AFID_ERR_NOMEM, "cudaMalloc(work arrays) failed"); return nullptr;
+        }
+    char* tb = (char*)pl->tables;
+    DevParams& d = pl->dp;
+    d.nx = nx; d.ny = ny; d.nz = nz; d.nzh = nh + 1;
+    d.rdy = (double)(1.0L / (ld)dy);
+    d.rdz = (double)(1.0L / (ld)dz);
+    d.spec_scale = (double)(-1.0L / ((ld)ny * (ld)nz));
+    d.rdx = (const double*)(tb + items[0].off);
+    d.rdc = (const double*)(tb + items[1].off);
+    d.dxw = (const double*)(tb + items[2].off);
+    d.ca = (const double*)(tb + items[3].off);
+    d.cc = (const double*)(tb + items[4].off);
+    d.lamy = (const double*)(tb + items[5].off);
+    d.lamz = (const double*)(tb + items[6].off);
+    d.tw_y = (const cplx*)(tb + items[7].off);
+    d.tw_zh = (const cplx*)(tb + items[8].off);
+    d.tw_z = (const cplx*)(tb + items[9].off);
+    d.inv_vol = (double)(1.0L / vol);
+    return pl;
+}
+
+int afid_plan_destroy(afid_plan* pl)
+{
+    if (!pl) return AFID_OK;
+    cudaFree(pl->ws[0]);
+    cudaFree(pl->ws[1]);
+    cudaFree(pl->tables);
+    delete pl;
+    return AFID_OK;
+}
+
+size_t afid_plan_workspace_bytes(const afid_plan* pl) { return pl ? 2 * pl->ws_bytes + pl->tables_bytes : 0; }
+int afid_plan_num_launches(const afid_plan* pl) { return pl ? 6 : 0; }
+
+static int launch(const LaunchCfg& c, unsigned grid, cudaStream_t st, void** args, const char* name)
+{
+    cudaError_t e = cudaLaunchKernel(c.fn, dim3(grid), dim3(c.threads), args, c.smem, st);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string(name) + ": " + cudaGetErrorString(e));
+    return AFID_OK;
+}
+
+static int check_ptr(const void* p, const char* name)
+{
+    if (!p) return fail(AFID_ERR_NULL, std::string(name) + " is NULL");
+    if (((size_t)p & 15) != 0) return fail(AFID_ERR_ALIGN, std::string(name) + " is not 16-byte aligned");
+    return AFID_OK;
+}
+
+// K1 + K2: u,v,w -> C layout spectrum in `outC`
+static int run_forward(afid_plan* pl, const double* u, const double* v, const double* w, cplx* wsB, cplx* outC, cudaStream_t st)
+{
+    int rc;
+    {
+        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB};
+        rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c");
+        if (rc) return rc;
+    }
+    {
+        void* args[] = {&pl->dp, (void*)&wsB, (void*)&outC};
+        rc = launch(pl->k2, (unsigned)(pl->nx * ((pl->nzh + KY_NL - 1) / KY_NL)), st, args, "k_fft_y");
+    }
+    return rc;
+}
+
+static int run_solve(afid_plan* pl, const cplx* inC, cplx* outT, cudaStream_t st)
+{
+    void* args[] = {&pl->dp, (void*)&inC, (void*)&outT};
+    return launch(pl->k3, (unsigned)(pl->nzh * (pl->ny / 8)), st, args, "k_solve_x");
+}
+
+int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void* stream)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    int rc;
+    if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(p, "p"))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = run_forward(pl, u, v, w, pl->ws[0], pl->ws[1], st))) return rc;   // B in ws0, C in ws1
+    if ((rc = run_solve(pl, pl->ws[1], pl->ws[0], st))) return rc;             // T in ws0
+    {
+        void* args[] = {&pl->dp, (void*)&pl->ws[0], (void*)&pl->ws[1]};          // D in ws1
+        if ((rc = launch(pl->k4, (unsigned)(pl->nzh * ((pl->nx + KY_NL - 1) / KY_NL)), st, args, "k_ifft_y"))) return rc;
+    }
+    {
+        void* args[] = {&pl->dp, (void*)&pl->ws[1], (void*)&p};
+        if ((rc = launch(pl->k5, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_z"))) return rc;
+    }
+    {
+        LaunchCfg c = {(const void*)k_correct, 256, 0};
+        void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w};
+        const size_t npair = (size_t)pl->nx * pl->ny * (pl->nz / 2);
+        size_t blocks = (npair + 255) / 256;
+        const size_t cap = (size_t)pl->n_sm * 64;
+        if (blocks > cap) blocks = cap;
+        if ((rc = launch(c, (unsigned)blocks, st, args, "k_correct"))) return rc;
+    }
+    return AFID_OK;
+}
+
+int afid_stage_forward(afid_plan* pl, const double* u, const double* v, const double* w, double* spec, void* stream)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    int rc;
+    if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(spec, "spec"))) return rc;
+    return run_forward(pl, u, v, w, pl->ws[0], (cplx*)spec, (cudaStream_t)stream);
+}
+
+// in place on a C-layout array: K3 writes the T layout into ws0, then a re-layout kernel is
+// not needed for the tap: K4's inverse transform is not part of this stage, so the tap
+// copies T back to C order with a small gather kernel.
+__global__ void k_tap_T_to_C(DevParams P, const cplx* __restrict__ T, cplx* __restrict__ C)
+{
+    const size_t n = (size_t)P.nx * P.nzh * P.ny;
+    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+        const int ky = (int)(t % P.ny);
+        const size_t r = t / P.ny;
+        const int kz = (int)(r % P.nzh), i = (int)(r / P.nzh);
+        C[t] = T[(((size_t)kz * (P.ny / 8) + ky / 8) * P.nx + i) * 8 + (ky & 7)];
+    }
+}
+
+int afid_stage_solve(afid_plan* pl, double* spec, void* stream)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    int rc;
+    if ((rc = check_ptr(spec, "spec"))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = run_solve(pl, (const cplx*)spec, pl->ws[0], st))) return rc;
+    k_tap_T_to_C<<<pl->n_sm * 8, 256, 0, st>>>(pl->dp, pl->ws[0], (cplx*)spec);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_tap_T_to_C: ") + cudaGetErrorString(e));
+    return AFID_OK;
+}
+
+} // extern "C"
