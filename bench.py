@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py -- fp64 projection throughput of the B200-native AFiD projection step.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4] [--impl reference]
+
+A "step" is one afid_project call (all six kernels) on one synthetic velocity field resident
+in HBM.  N = 1 runs BASELINE.json's headline configuration C4 (1024 x 1536 x 1536, tanh grid);
+N > 1 (under torchrun) runs N independent replicas, one per GPU ("replicas only": the path
+does not shard without a transpose), value = total points / max-over-ranks time.
+Prints ONE JSON line on rank 0.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload: it is a deliberately slow baseline, not a target.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 projection Mpoints/s at 1024x1536x1536; % of B200 HBM roofline"
+UNIT = "Mpoints/s"
+# algorithmic HBM bytes per grid point of each kernel: fp64, complex = 16 B per 2 points
+ALG_BYTES_PER_POINT = {"k_div_r2c": 32.0, "k_fft_y": 16.0, "k_solve_x": 16.0, "k_ifft_y": 16.0, "k_c2r_z": 16.0,
+                       "k_correct": 56.0}
+PATH_ALG_BYTES_PER_POINT = 96.0   # strict minimum of the whole path
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "about 8 TB/s"
+
+
+def rank_info():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def is_printing_rank():
+    return rank_info()[0] == 0
+
+
+def aggregate_over_ranks(ms, points, device="cuda"):
+    """(max over ranks of ms, sum over ranks of points); identity when not distributed."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms), int(points)
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    n = torch.tensor([int(points)], dtype=torch.int64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(n.item())
+
+
+def make_line(config, n_gpus, steps, warmup, ms_total, points_per_step, **extra):
+    ms_per_step = ms_total / steps
+    line = {"metric": METRIC, "value": points_per_step / (ms_per_step * 1e-3) / 1e6, "unit": UNIT, "n_gpus": n_gpus,
+            "steps": steps, "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config}
+    line.update(extra)
+    return line
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+def ncu_traffic(kernel):
+    """DRAM bytes per launch of `kernel` at C4 from the committed ncu capture, or None."""
+    path = os.path.join(ROOT, "profiles", "r1_c4_dram_traffic.csv")
+    try:
+        with open(path) as f:
+            for ln in f:
+                parts = ln.strip().split(",")
+                if parts and parts[0] == kernel:
+                    return float(parts[1]) + float(parts[2])
+    except Exception:
+        pass
+    return None
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons of one GPU during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.rows.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def run_gpu(args):
+    import torch
+    import paper_1705_01423_b200 as afid
+    from paper_1705_01423_b200 import synth
+
+    rank, local_rank, world = rank_info()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = synth.config(args.workload)
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    N = nx * ny * nz
+    xc = synth.grid_faces(cfg)
+    plan = afid.Plan(nx, ny, nz, xc, cfg["Ly"], cfg["Lz"])
+    u = torch.empty((nx + 1, ny, nz), dtype=torch.float64, device=dev)
+    v = torch.empty((nx, ny, nz), dtype=torch.float64, device=dev)
+    w = torch.empty_like(v)
+    p = torch.empty_like(v)
+    synth.velocity(cfg, xc, device=dev, out=(u, v, w))     # seeded synthetic field, generated on the device
+    torch.cuda.synchronize()
+    plan.enable_timing(True)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        plan.project(u, v, w, p)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kt = {}
+    e0.record(stream)
+    for _ in range(args.steps):
+        plan.project(u, v, w, p)
+    e1.record(stream)
+    barrier()
+    ms_local = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    # per-kernel durations (CUDA events recorded by the library on the same stream; the last
+    # step's are read here, then averaged over a few more steps outside the timed region)
+    acc = {}
+    reps = max(1, min(args.steps, 3))
+    for k, t in plan.kernel_times().items():
+        acc[k] = t
+    for _ in range(reps - 1):
+        plan.project(u, v, w, p)
+        for k, t in plan.kernel_times().items():
+            acc[k] += t
+    kt = {k: t / reps for k, t in acc.items()}
+    ms_total, pts = aggregate_over_ranks(ms_local, N, device=dev)
+
+    # end to end through the C ABI with HOST buffers: H2D of u,v,w, project, D2H of u,v,w,p per step
+    e2e = None
+    if not args.no_e2e:
+        try:
+            hu = torch.empty(u.shape, dtype=torch.float64, pin_memory=True)
+            hv = torch.empty(v.shape, dtype=torch.float64, pin_memory=True)
+            hw = torch.empty(v.shape, dtype=torch.float64, pin_memory=True)
+            hp = torch.empty(v.shape, dtype=torch.float64, pin_memory=True)
+            synth.velocity(cfg, xc, device=dev, out=(u, v, w))
+            hu.copy_(u); hv.copy_(v); hw.copy_(w)
+            torch.cuda.synchronize()
+            es = max(1, args.e2e_steps)
+            barrier()
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record(stream)
+            for _ in range(es):
+                u.copy_(hu, non_blocking=True); v.copy_(hv, non_blocking=True); w.copy_(hw, non_blocking=True)
+                plan.project(u, v, w, p)
+                hu.copy_(u, non_blocking=True); hv.copy_(v, non_blocking=True); hw.copy_(w, non_blocking=True)
+                hp.copy_(p, non_blocking=True)
+            a1.record(stream)
+            barrier()
+            ms_e, pts_e = aggregate_over_ranks(a0.elapsed_time(a1), N, device=dev)
+            bi = (u.numel() + v.numel() + w.numel()) * 8
+            bo = bi + p.numel() * 8
+            e2e = {"value": pts_e / (ms_e / es * 1e-3) / 1e6, "unit": UNIT, "steps": es, "ms_per_step": ms_e / es,
+                   "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo, "host_memory": "pinned"}
+            del hu, hv, hw, hp
+        except Exception as ex:  # pinned allocation can fail on small hosts
+            e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
+
+    peak, peak_src = measured_peaks()
+    dom = max(kt, key=kt.get)
+    ach = ALG_BYTES_PER_POINT[dom] * N / (kt[dom] * 1e-3) / 1e9
+    traffic = ncu_traffic(dom) if args.workload == "C4" else None
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": traffic, "peak_source": peak_src,
+                "alg_bytes_per_launch": ALG_BYTES_PER_POINT[dom] * N, "kernel_ms": kt[dom]}
+    ms_step = ms_total / args.steps
+    path_gbs = PATH_ALG_BYTES_PER_POINT * N / (ms_local / args.steps * 1e-3) / 1e9
+    kernels = {k: {"ms": t, "alg_GBps": ALG_BYTES_PER_POINT[k] * N / (t * 1e-3) / 1e9,
+                   "frac_of_peak": ALG_BYTES_PER_POINT[k] * N / (t * 1e-3) / 1e9 / peak} for k, t in kt.items()}
+    config = {"workload": f"{args.workload}: {nx}x{ny}x{nz} {cfg['grid']}-clustered x grid, Ly={cfg['Ly']:.6g}, "
+                          f"Lz={cfg['Lz']:.6g}, seeded random-mode velocity (synth.py)",
+              "points_per_step_per_gpu": N, "parallelism": "replicas only" if world > 1 else "1 gpu",
+              "l2": "working set (>= 77 GB) far larger than the 126 MB L2; no flush needed",
+              "device_bytes": plan.workspace_bytes + (4 * N + ny * nz) * 8}
+    line = make_line(config, world, args.steps, args.warmup, ms_total, pts, clocks=clocks, e2e=e2e,
+                     gpu_launches=plan.num_launches * args.steps, roofline=roofline, kernels=kernels,
+                     path_roofline={"alg_bytes_per_point": PATH_ALG_BYTES_PER_POINT, "achieved_GBps": path_gbs,
+                                    "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS, "frac_of_measured": path_gbs / peak})
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(args.workload)
+    elif rank == 0:
+        line["cpu_baseline"] = None
+    plan.destroy()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ------------------------------------------------------------------------------------------
+def oracle_sample(workload):
+    """The bounded sample: a slab of nx=2 cells with the workload's full y-z cross-section (the
+    per-point cost of the oracle's naive DFT, O(ny+nz), is that of the full workload)."""
+    from paper_1705_01423_b200 import synth
+    cfg = synth.config(workload, nx=2)
+    xc = synth.grid_faces(synth.config(workload))[:3].copy()
+    u, v, w = synth.velocity(cfg, xc)
+    desc = f"{workload} cross-section slab: nx=2 x ny={cfg['ny']} x nz={cfg['nz']} (first two cells of the x grid)"
+    return cfg, xc, u.numpy(), v.numpy(), w.numpy(), desc
+
+
+def time_oracle(cfg, xc, u, v, w):
+    from oracle import ref
+    t0 = time.perf_counter()
+    ref.project(xc, cfg["Ly"], cfg["Lz"], u, v, w)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(workload):
+    from oracle import ref
+    cfg, xc, u, v, w, desc = oracle_sample(workload)
+    dt = time_oracle(cfg, xc, u, v, w)
+    n = cfg["nx"] * cfg["ny"] * cfg["nz"]
+    return {"value": n / dt / 1e6, "unit": UNIT, "cores": ref.num_threads(), "kind": "oracle",
+            "sample": desc + f"; one oracle projection, {dt:.1f} s"}
+
+
+def run_reference(args):
+    rank, _, world = rank_info()
+    if rank != 0:
+        return
+    from oracle import ref
+    from paper_1705_01423_b200 import synth
+    cfg, xc, u, v, w, desc = oracle_sample(args.workload)
+    n = cfg["nx"] * cfg["ny"] * cfg["nz"]
+    for _ in range(args.warmup):
+        time_oracle(cfg, xc, u, v, w)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        time_oracle(cfg, xc, u, v, w)
+    ms_total = (time.perf_counter() - t0) * 1e3
+    full = synth.config(args.workload)
+    config = {"workload": f"{args.workload}: {full['nx']}x{full['ny']}x{full['nz']} (each step = bounded sample: {desc})"}
+    line = make_line(config, world, args.steps, args.warmup, ms_total, n, impl="reference")
+    line["gpu_launches"] = 0
+    line["cpu_baseline"] = {"value": line["value"], "unit": UNIT, "cores": ref.num_threads(), "kind": "oracle", "sample": desc}
+    line["e2e"] = {"value": line["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 2 if args.steps is None else args.steps
+        args.warmup = 1 if args.warmup is None else args.warmup
+        run_reference(args)
+    else:
+        args.steps = 10 if args.steps is None else args.steps
+        args.warmup = 3 if args.warmup is None else max(3, args.warmup)
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -87,6 +87,17 @@ size_t afid_plan_workspace_bytes(const afid_plan* plan);
 int afid_plan_num_launches(const afid_plan* plan);
 
 /*
+ * Per-kernel device timing, for the roofline report.  With timing enabled afid_project
+ * records a CUDA event on `stream` before and after each of its kernels (no host sync).
+ * afid_plan_kernel_times synchronises on the last recorded event and writes the duration in
+ * milliseconds of each kernel of the most recent afid_project call into ms[0..n-1]
+ * (HOST pointer, n <= afid_plan_num_launches); afid_plan_kernel_name gives their names.
+ */
+int afid_plan_enable_timing(afid_plan* plan, int on);
+int afid_plan_kernel_times(afid_plan* plan, float* ms, int n);
+const char* afid_plan_kernel_name(const afid_plan* plan, int k);
+
+/*
  * Stage taps, for stage-wise parity tests (same kernels as afid_project, run separately):
  *   afid_stage_forward:  u,v,w -> spectrum of -(div u)/(ny*nz), written to `spec`
  *                        (DEVICE, nx*(nz/2+1)*ny complex doubles, layout [i][kz][ky]).

@@ -21,7 +21,8 @@ ERRORS = {-1: "AFID_ERR_NULL", -2: "AFID_ERR_ALIGN", -3: "AFID_ERR_UNSUPPORTED_S
 # every symbol include/afid.h declares
 SYMBOLS = ["afid_plan_create", "afid_project", "afid_plan_destroy", "afid_plan_workspace_bytes",
            "afid_plan_num_launches", "afid_stage_forward", "afid_stage_solve", "afid_fft_length_supported",
-           "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version"]
+           "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version",
+           "afid_plan_enable_timing", "afid_plan_kernel_times", "afid_plan_kernel_name"]
 
 _lib = None
 
@@ -61,6 +62,12 @@ def lib():
         L.afid_last_error.restype = C.c_char_p
         L.afid_last_error_code.restype = i
         L.afid_version.restype = C.c_char_p
+        L.afid_plan_enable_timing.restype = i
+        L.afid_plan_enable_timing.argtypes = [vp, i]
+        L.afid_plan_kernel_times.restype = i
+        L.afid_plan_kernel_times.argtypes = [vp, vp, i]
+        L.afid_plan_kernel_name.restype = C.c_char_p
+        L.afid_plan_kernel_name.argtypes = [vp, i]
         _lib = L
     return _lib
 
@@ -143,6 +150,17 @@ class Plan:
         """afid_stage_solve: in-place x-solves on a [i][kz][ky] spectrum."""
         m = 2 * self.nx * self.nzh * self.ny
         _check(lib().afid_stage_solve(self._h, _dev_ptr(spec, m, "spec"), self._stream(stream)))
+
+    def enable_timing(self, on=True):
+        """afid_plan_enable_timing: record CUDA events around each kernel of project()."""
+        _check(lib().afid_plan_enable_timing(self._h, 1 if on else 0))
+
+    def kernel_times(self):
+        """afid_plan_kernel_times: {kernel name: ms} of the most recent project() (synchronises)."""
+        n = self.num_launches
+        ms = (C.c_float * n)()
+        _check(lib().afid_plan_kernel_times(self._h, C.cast(ms, C.c_void_p), n))
+        return {lib().afid_plan_kernel_name(self._h, k).decode(): float(ms[k]) for k in range(n)}
 
     def destroy(self):
         if getattr(self, "_h", None):

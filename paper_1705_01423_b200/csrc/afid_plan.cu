@@ -107,9 +107,14 @@ struct afid_plan {
     cplx* ws[2];       // work arrays, nx*nzh*ny complex each
     size_t ws_bytes;
     LaunchCfg k1, k2, k4, k5, k3;
-    int k3_threads;
     int n_sm;
+    // optional per-kernel timing (afid_plan_enable_timing): NK+1 events around the NK kernels
+    bool timing;
+    cudaEvent_t ev[7];
+    bool ev_valid;
 };
+
+static const char* const KERNEL_NAMES[6] = {"k_div_r2c", "k_fft_y", "k_solve_x", "k_ifft_y", "k_c2r_z", "k_correct"};
 
 extern "C" {
 
@@ -243,6 +248,8 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
 int afid_plan_destroy(afid_plan* pl)
 {
     if (!pl) return AFID_OK;
+    if (pl->timing)
+        for (int k = 0; k < 7; ++k) cudaEventDestroy(pl->ev[k]);
     cudaFree(pl->ws[0]);
     cudaFree(pl->ws[1]);
     cudaFree(pl->tables);
@@ -295,16 +302,32 @@ int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void
     int rc;
     if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(p, "p"))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    if ((rc = run_forward(pl, u, v, w, pl->ws[0], pl->ws[1], st))) return rc;   // B in ws0, C in ws1
+    const bool tm = pl->timing;
+    cplx* wsB = pl->ws[0];
+    cplx* wsC = pl->ws[1];
+    if (tm) cudaEventRecord(pl->ev[0], st);
+    {
+        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB};   // B in ws0
+        if ((rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c"))) return rc;
+    }
+    if (tm) cudaEventRecord(pl->ev[1], st);
+    {
+        void* args[] = {&pl->dp, (void*)&wsB, (void*)&wsC};                        // C in ws1
+        if ((rc = launch(pl->k2, (unsigned)(pl->nx * ((pl->nzh + KY_NL - 1) / KY_NL)), st, args, "k_fft_y"))) return rc;
+    }
+    if (tm) cudaEventRecord(pl->ev[2], st);
     if ((rc = run_solve(pl, pl->ws[1], pl->ws[0], st))) return rc;             // T in ws0
+    if (tm) cudaEventRecord(pl->ev[3], st);
     {
         void* args[] = {&pl->dp, (void*)&pl->ws[0], (void*)&pl->ws[1]};          // D in ws1
         if ((rc = launch(pl->k4, (unsigned)(pl->nzh * ((pl->nx + KY_NL - 1) / KY_NL)), st, args, "k_ifft_y"))) return rc;
     }
+    if (tm) cudaEventRecord(pl->ev[4], st);
     {
         void* args[] = {&pl->dp, (void*)&pl->ws[1], (void*)&p};
         if ((rc = launch(pl->k5, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_z"))) return rc;
     }
+    if (tm) cudaEventRecord(pl->ev[5], st);
     {
         LaunchCfg c = {(const void*)k_correct, 256, 0};
         void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w};
@@ -314,7 +337,40 @@ int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void
         if (blocks > cap) blocks = cap;
         if ((rc = launch(c, (unsigned)blocks, st, args, "k_correct"))) return rc;
     }
+    if (tm) { cudaEventRecord(pl->ev[6], st); pl->ev_valid = true; }
     return AFID_OK;
+}
+
+int afid_plan_enable_timing(afid_plan* pl, int on)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    if (on && !pl->timing) {
+        for (int k = 0; k < 7; ++k)
+            if (cudaEventCreate(&pl->ev[k]) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventCreate failed");
+        pl->timing = true;
+        pl->ev_valid = false;
+    } else if (!on && pl->timing) {
+        for (int k = 0; k < 7; ++k) cudaEventDestroy(pl->ev[k]);
+        pl->timing = false;
+        pl->ev_valid = false;
+    }
+    return AFID_OK;
+}
+
+int afid_plan_kernel_times(afid_plan* pl, float* ms, int n)
+{
+    if (!pl || !ms) return fail(AFID_ERR_NULL, "plan or ms is NULL");
+    if (!pl->timing || !pl->ev_valid) return fail(AFID_ERR_CUDA, "timing not enabled or no projection recorded");
+    if (cudaEventSynchronize(pl->ev[6]) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventSynchronize failed");
+    for (int k = 0; k < 6 && k < n; ++k)
+        if (cudaEventElapsedTime(&ms[k], pl->ev[k], pl->ev[k + 1]) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventElapsedTime failed");
+    return AFID_OK;
+}
+
+const char* afid_plan_kernel_name(const afid_plan* pl, int k)
+{
+    (void)pl;
+    return (k >= 0 && k < 6) ? KERNEL_NAMES[k] : "";
 }
 
 int afid_stage_forward(afid_plan* pl, const double* u, const double* v, const double* w, double* spec, void* stream)

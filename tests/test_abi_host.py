@@ -1,0 +1,94 @@
+"""Host-side checks that need no GPU: the C-ABI library builds and loads, exports every symbol
+include/afid.h declares, fails loudly without a device, and the product never touches oracle/."""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "afid.h")
+
+
+@pytest.fixture(scope="module")
+def built_lib():
+    from paper_1705_01423_b200 import build
+    return build.build()
+
+
+def declared_symbols():
+    txt = open(HEADER).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(afid_[a-z0-9_]+)\s*\(", txt)))
+
+
+def test_header_declares_the_boundary_calls():
+    syms = declared_symbols()
+    for name in ("afid_plan_create", "afid_project", "afid_plan_destroy"):
+        assert name in syms
+
+
+def test_library_exports_every_declared_symbol(built_lib):
+    lib = ctypes.CDLL(built_lib)
+    for name in declared_symbols():
+        assert hasattr(lib, name), name
+    import paper_1705_01423_b200 as afid
+    assert sorted(afid.SYMBOLS) == declared_symbols()
+    assert b"sm_100a" in ctypes.cast(afid.lib().afid_version, ctypes.CFUNCTYPE(ctypes.c_char_p))()
+
+
+def test_library_is_sm100a_only(built_lib):
+    out = subprocess.run(["cuobjdump", "-lelf", built_lib], capture_output=True, text=True).stdout
+    archs = set(re.findall(r"sm_(\d+a?)", out))
+    assert archs == {"100a"}, archs
+
+
+def test_supported_sizes_host_queries(built_lib):
+    import paper_1705_01423_b200 as afid
+    for n in (16, 32, 128, 256, 512, 768, 1024, 1536, 4096):
+        assert afid.fft_length_supported(n), n
+    for n in (0, 7, 15, 40, 100, 1000, 5000):
+        assert not afid.fft_length_supported(n), n
+    assert afid.max_nx() >= 1024
+
+
+def test_no_cpu_fallback_without_device(built_lib):
+    """On a box without a GPU plan creation must fail with an error, not fall back."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    import paper_1705_01423_b200 as afid
+    with pytest.raises(afid.AfidError) as e:
+        afid.Plan(32, 32, 32, np.linspace(0.0, 1.0, 33), 1.0, 1.0)
+    assert e.value.code == -6
+    # argument validation happens before the device is touched
+    with pytest.raises(afid.AfidError) as e:
+        afid.Plan(32, 40, 32, np.linspace(0.0, 1.0, 33), 1.0, 1.0)
+    assert e.value.code == -3
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1705_01423_b200")
+    pat = re.compile(r"^\s*(from|import)\s+oracle\b|libafid_ref|afid_ref\.c|#include\s+\".*oracle", re.M)
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                assert not pat.search(open(os.path.join(dirpath, f)).read()), (dirpath, f)
+    for f in ("afid_ref.c", "ref.py", "build.py"):
+        src = open(os.path.join(ROOT, "oracle", f)).read()
+        assert "import paper_1705_01423_b200" not in src and "libafid_b200" not in src and "#include \"afid" not in src
+
+
+def test_bench_rank_aggregation_gloo_world2():
+    """N>1 path of bench.py = independent replicas; its only cross-rank step is the max-over-
+    ranks of the device time and the sum of points.  Run it on 2 CPU ranks over gloo."""
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    res = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29631",
+                          os.path.join(ROOT, "tests", "gloo_worker.py")],
+                         capture_output=True, text=True, env=env, timeout=600)
+    assert res.returncode == 0, res.stderr[-2000:]
+    assert "gloo_worker ok rank 0" in res.stdout and "gloo_worker ok rank 1" in res.stdout

@@ -1,0 +1,263 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, element by
+element on the same seeded inputs, plus the full-size checks of the bench configurations.
+
+Tolerances (BASELINE.json north_star): relative L2 <= 1e-11 in p and in the corrected u, v, w;
+post-projection max|div| <= 1e-10 * max|div_in|.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import paper_1705_01423_b200 as afid
+from paper_1705_01423_b200 import synth
+from oracle import ref
+
+import manufactured as mf
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+DIV_TOL = 1e-10
+
+
+def rel(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+def gpu_project(cfg, xc, u, v, w, calls=1):
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    plan = afid.Plan(nx, ny, nz, xc, cfg["Ly"], cfg["Lz"])
+    ud, vd, wd = u.cuda(), v.cuda(), w.cuda()
+    p = torch.full((nx, ny, nz), float("nan"), dtype=torch.float64, device="cuda")
+    outs = []
+    for _ in range(calls):
+        plan.project(ud, vd, wd, p)
+        torch.cuda.synchronize()
+        outs.append((ud.cpu().numpy().copy(), vd.cpu().numpy().copy(), wd.cpu().numpy().copy(), p.cpu().numpy().copy()))
+    plan.destroy()
+    return outs
+
+
+def check_against_oracle(cfg, xc, u, v, w):
+    un, vn, wn = u.numpy(), v.numpy(), w.numpy()
+    uo, vo, wo, po, max_imag = ref.project(xc, cfg["Ly"], cfg["Lz"], un, vn, wn)
+    ug, vg, wg, pg = gpu_project(cfg, xc, u, v, w)[0]
+    errs = dict(p=rel(pg, po), u=rel(ug, uo), v=rel(vg, vo), w=rel(wg, wo))
+    assert all(e <= TOL for e in errs.values()), errs
+    # invariants on the GPU output, evaluated with the oracle's operators
+    din = np.abs(ref.divergence(xc, cfg["Ly"], cfg["Lz"], un, vn, wn)).max()
+    dout = np.abs(ref.divergence(xc, cfg["Ly"], cfg["Lz"], ug, vg, wg)).max()
+    assert dout <= DIV_TOL * din, (dout, din)
+    dx = np.diff(xc)
+    mean = (pg * dx[:, None, None]).sum() / (dx.sum() * cfg["ny"] * cfg["nz"])
+    assert abs(mean) <= 1e-13 * np.abs(pg).max()
+    nx = cfg["nx"]
+    assert np.array_equal(ug[0], un[0]) and np.array_equal(ug[nx], un[nx])  # wall planes bit-unchanged
+    return errs
+
+
+def test_c1_parity():
+    cfg = synth.config("C1")
+    xc = synth.grid_faces(cfg)
+    u, v, w = synth.velocity(cfg, xc)
+    check_against_oracle(cfg, xc, u, v, w)
+
+
+# odd shapes: radix-3 lengths, ny != nz, ragged last x-chunk (nx % 16 != 0, nx % 4 != 0),
+# the three K3 instantiations (nx < 64, <= 1024, > 1024), minimum sizes
+SHAPES = [
+    dict(nx=2, ny=8, nz=16, grid="uniform"),
+    dict(nx=5, ny=24, nz=48, grid="tanh", s=3.0, Ly=1.3, Lz=0.7),
+    dict(nx=63, ny=32, nz=64, grid="tanh", s=3.0),
+    dict(nx=65, ny=96, nz=64, grid="tanh", s=3.0, Ly=2.0, Lz=0.5),
+    dict(nx=33, ny=192, nz=384, grid="erf", s=1.5, x_lo=-1.0, x_hi=1.0, Ly=8 * math.pi, Lz=2 * math.pi, shear=1.0),
+    dict(nx=100, ny=48, nz=96, grid="tanh", s=3.0),
+    dict(nx=1030, ny=8, nz=32, grid="tanh", s=3.0),
+    dict(nx=40, ny=64, nz=128, grid="tanh", s=3.0, M=32, expo=-5.0 / 6.0),
+    dict(nx=17, ny=128, nz=256, grid="uniform"),
+    dict(nx=16, ny=384, nz=192, grid="tanh", s=3.0),
+]
+
+
+@pytest.mark.parametrize("ov", SHAPES, ids=lambda o: f"{o['nx']}x{o['ny']}x{o['nz']}")
+def test_shapes_parity(ov):
+    cfg = synth.config("C1", **ov)
+    xc = synth.grid_faces(cfg)
+    u, v, w = synth.velocity(cfg, xc)
+    check_against_oracle(cfg, xc, u, v, w)
+
+
+def test_stage_taps_parity():
+    """Forward spectrum and x-solve separately (stage boundaries of the paper's step list)."""
+    cfg = synth.config("C1", nx=37, ny=48, nz=96, grid="tanh", s=3.0, Ly=1.5, Lz=0.75)
+    xc = synth.grid_faces(cfg)
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    nzh = nz // 2 + 1
+    u, v, w = synth.velocity(cfg, xc)
+    d = ref.divergence(xc, cfg["Ly"], cfg["Lz"], u.numpy(), v.numpy(), w.numpy())
+    dh = ref.forward_spectrum(d)                       # [nx][ny][nz], unnormalised
+    want_fwd = -dh[:, :, :nzh].transpose(0, 2, 1) / (ny * nz)
+    plan = afid.Plan(nx, ny, nz, xc, cfg["Ly"], cfg["Lz"])
+    spec = torch.zeros(2 * nx * nzh * ny, dtype=torch.float64, device="cuda")
+    plan.stage_forward(u.cuda(), v.cuda(), w.cuda(), spec)
+    torch.cuda.synchronize()
+    got = spec.cpu().numpy().view(np.complex128).reshape(nx, nzh, ny)
+    assert rel(got, want_fwd) <= 1e-13
+    xs = ref.solve(xc, cfg["Ly"], cfg["Lz"], dh)       # oracle solves a x - (a+c+lam) x + c x = dhat
+    want_sol = xs[:, :, :nzh].transpose(0, 2, 1) / (ny * nz)
+    spec2 = torch.from_numpy(np.ascontiguousarray(want_fwd).view(np.float64).ravel().copy()).cuda()
+    plan.stage_solve(spec2)
+    torch.cuda.synchronize()
+    got2 = spec2.cpu().numpy().view(np.complex128).reshape(nx, nzh, ny)
+    assert rel(got2, want_sol) <= 1e-13
+    assert np.abs(got2[:, 0, 0] - want_sol[:, 0, 0]).max() <= 1e-13 * np.abs(want_sol[:, 0, 0]).max()
+    plan.destroy()
+
+
+def test_idempotent_and_back_to_back():
+    """C2-shaped (reduced in y,z so the oracle takes seconds): parity on call 1, a second
+    projection of the projected field changes nothing beyond round-off (invariant P4 iii)."""
+    cfg = synth.config("C2", ny=64, nz=64)
+    xc = synth.grid_faces(cfg)
+    u, v, w = synth.velocity(cfg, xc)
+    check_against_oracle(cfg, xc, u, v, w)
+    (u1, v1, w1, p1), (u2, v2, w2, p2) = gpu_project(cfg, xc, u, v, w, calls=2)
+    assert np.linalg.norm(p2) <= 1e-10 * np.linalg.norm(p1)
+    assert rel(u2, u1) <= 1e-12 and rel(v2, v1) <= 1e-12 and rel(w2, w1) <= 1e-12
+
+
+def test_c2_full_parity():
+    """BASELINE config 2 at full size (256^3, tanh grid) against the full oracle."""
+    cfg = synth.config("C2")
+    xc = synth.grid_faces(cfg)
+    u, v, w = synth.velocity(cfg, xc)
+    check_against_oracle(cfg, xc, u, v, w)
+
+
+def test_error_codes():
+    xc = np.linspace(0.0, 1.0, 33)
+    with pytest.raises(afid.AfidError) as e:
+        afid.Plan(32, 40, 32, xc, 1.0, 1.0)           # 40 is not a supported FFT length
+    assert e.value.code == -3
+    with pytest.raises(afid.AfidError) as e:
+        afid.Plan(32, 32, 30, xc, 1.0, 1.0)           # nz/2 = 15
+    assert e.value.code == -3
+    bad = xc.copy()
+    bad[5] = bad[4]
+    with pytest.raises(afid.AfidError) as e:
+        afid.Plan(32, 32, 32, bad, 1.0, 1.0)
+    assert e.value.code == -4
+    with pytest.raises(afid.AfidError) as e:
+        afid.Plan(32, 32, 32, xc, -1.0, 1.0)
+    assert e.value.code == -4
+    with pytest.raises(afid.AfidError) as e:
+        afid.Plan(afid.max_nx() + 1, 32, 32, np.linspace(0, 1, afid.max_nx() + 2), 1.0, 1.0)
+    assert e.value.code == -3
+    plan = afid.Plan(32, 32, 32, xc, 1.0, 1.0)
+    n = 32 ** 3
+    big = torch.zeros(n + 32 * 32 + 1, dtype=torch.float64, device="cuda")
+    v = torch.zeros(n, dtype=torch.float64, device="cuda")
+    with pytest.raises(afid.AfidError) as e:            # u shifted by 8 bytes: misaligned
+        plan.project(big[1:], v, v.clone(), v.clone())
+    assert e.value.code == -2
+    plan.destroy()
+
+
+# ---------------------------------------------------------------------------------------
+# Full-size configurations (C3, C4 = the bench workload, C5): the oracle's O(N (ny+nz)) DFT
+# cannot run there, so (a) a manufactured Helmholtz split whose exact answer is known by
+# construction, (b) the invariants, (c) oracle-computed samples of the forward spectrum.
+# ---------------------------------------------------------------------------------------
+def _full_size_checks(name, sample_planes):
+    cfg = synth.config(name)
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    nzh = nz // 2 + 1
+    need = (4 * nx * ny * nz * 8 + 2 * nx * nzh * ny * 16) * 1.35
+    free, _ = torch.cuda.mem_get_info()
+    if free < need:
+        pytest.skip(f"{name} needs {need / 2**30:.0f} GiB of device memory")
+    xc = synth.grid_faces(cfg)
+    dev = "cuda"
+    u = torch.empty((nx + 1, ny, nz), dtype=torch.float64, device=dev)
+    v = torch.empty((nx, ny, nz), dtype=torch.float64, device=dev)
+    w = torch.empty_like(v)
+    phi, psi, chi = mf.potentials(cfg, xc, dev)
+    mf.solenoidal_into(cfg, xc, psi, chi, u, v, w)
+    mf.add_gradient(cfg, xc, phi, u, v, w)
+    del phi, psi, chi
+    torch.cuda.empty_cache()
+    div_in = mf.max_abs_divergence(cfg, xc, u, v, w)
+    wall0, wall1 = u[0].clone(), u[nx].clone()
+
+    plan = afid.Plan(nx, ny, nz, xc, cfg["Ly"], cfg["Lz"])
+    # (c) sampled forward spectrum against the oracle's naive DFT of the oracle's divergence
+    if sample_planes:
+        spec = torch.empty(2 * nx * nzh * ny, dtype=torch.float64, device=dev)
+        plan.stage_forward(u, v, w, spec)
+        torch.cuda.synchronize()
+        sg = spec.view(nx, nzh, ny, 2)
+        for i in sample_planes:
+            i = min(i, nx - 2)
+            d2 = ref.divergence(xc[i:i + 3], cfg["Ly"], cfg["Lz"], u[i:i + 3].cpu().numpy(),
+                                v[i:i + 2].cpu().numpy(), w[i:i + 2].cpu().numpy())
+            dh = ref.forward_spectrum(d2[:1])[0]        # [ny][nz]
+            want = -dh[:, :nzh].T / (ny * nz)           # [kz][ky]
+            got = sg[i].cpu().numpy().view(np.complex128).reshape(nzh, ny)
+            assert rel(got, want) <= 1e-12, (name, i, rel(got, want))
+        del spec, sg
+        torch.cuda.empty_cache()
+    p = torch.full((nx, ny, nz), float("nan"), dtype=torch.float64, device=dev)
+    plan.project(u, v, w, p)
+    torch.cuda.synchronize()
+    plan.destroy()
+    torch.cuda.empty_cache()
+
+    # (b) invariants
+    div_out = mf.max_abs_divergence(cfg, xc, u, v, w)
+    assert div_out <= DIV_TOL * div_in, (div_out, div_in)
+    assert torch.equal(u[0], wall0) and torch.equal(u[nx], wall1)
+    dx = torch.as_tensor(np.diff(xc)).to(dev)
+    wsum = sum(float(p[i].sum()) * float(dx[i]) for i in range(nx))
+    assert abs(wsum / (float(dx.sum()) * ny * nz)) <= 1e-13 * float(p.abs().max())
+    # (a) exact answer by construction
+    phi, psi, chi = mf.potentials(cfg, xc, dev)
+    e_p = mf.rel_l2(p, phi)
+    del p
+    torch.cuda.empty_cache()
+    us = torch.empty_like(u)
+    mf.solenoidal_into(cfg, xc, psi, chi, us, phi, psi)   # v_sol -> phi's storage, w_sol -> psi's storage
+    e_u, e_v, e_w = mf.rel_l2(u, us), mf.rel_l2(v, phi), mf.rel_l2(w, psi)
+    assert max(e_p, e_u, e_v, e_w) <= TOL, dict(p=e_p, u=e_u, v=e_v, w=e_w)
+
+
+def test_manufactured_small():
+    """The same construction on a size the oracle handles: both must agree with the known answer."""
+    cfg = synth.config("C2", nx=48, ny=32, nz=64)
+    xc = synth.grid_faces(cfg)
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    u = torch.empty((nx + 1, ny, nz), dtype=torch.float64)
+    v = torch.empty((nx, ny, nz), dtype=torch.float64)
+    w = torch.empty_like(v)
+    phi, psi, chi = mf.potentials(cfg, xc, "cpu")
+    mf.solenoidal_into(cfg, xc, psi, chi, u, v, w)
+    us, vs, ws = u.clone(), v.clone(), w.clone()
+    mf.add_gradient(cfg, xc, phi, u, v, w)
+    uo, vo, wo, po, _ = ref.project(xc, cfg["Ly"], cfg["Lz"], u.numpy(), v.numpy(), w.numpy())
+    assert rel(po, phi.numpy()) <= 1e-12 and rel(uo, us.numpy()) <= 1e-12
+    ug, vg, wg, pg = gpu_project(cfg, xc, u, v, w)[0]
+    assert rel(pg, phi.numpy()) <= TOL and rel(ug, us.numpy()) <= TOL
+    assert rel(vg, vs.numpy()) <= TOL and rel(wg, ws.numpy()) <= TOL
+
+
+def test_c3_full_size():
+    _full_size_checks("C3", sample_planes=[0, 300])
+
+
+def test_c4_full_size_bench_workload():
+    _full_size_checks("C4", sample_planes=[511])
+
+
+def test_c5_full_size():
+    _full_size_checks("C5", sample_planes=[383])
