@@ -49,7 +49,8 @@ typedef struct afid_plan afid_plan; /* opaque; owned by the library */
  * afid_plan_create -- build a plan for an nx x ny x nz grid on the CURRENT CUDA device.
  *   nx      cells in x, 2 <= nx <= afid_max_nx()
  *   ny, nz  periodic cells; ny and nz/2 must be lengths the FFT kernels are instantiated
- *           for (afid_fft_length_supported): powers of two times 1 or 3, 8..4096
+ *           for (afid_fft_length_supported, afid_fft_half_length_supported): powers of two
+ *           times 1 or 3, ny in 8..4096, nz/2 in 8..1024
  *   xc      HOST pointer, nx+1 face coordinates (copied; caller keeps ownership)
  *   Ly, Lz  periodic box lengths (> 0)
  * The plan owns: reciprocal metrics, tridiagonal coefficients a_i, c_i, modified
@@ -108,8 +109,10 @@ int afid_stage_forward(afid_plan* plan, const double* u, const double* v, const 
                        double* spec, void* stream);
 int afid_stage_solve(afid_plan* plan, double* spec, void* stream);
 
-/* 1 if the FFT kernels are instantiated for complex length n (ny must satisfy this, and nz/2). */
+/* 1 if the y-direction FFT kernels are instantiated for complex length n (ny must satisfy this). */
 int afid_fft_length_supported(int n);
+/* 1 if the z-direction (real-data) FFT kernels are instantiated for half length n (nz/2 must satisfy this). */
+int afid_fft_half_length_supported(int n);
 /* Largest nx the tridiagonal kernel supports. */
 int afid_max_nx(void);
 

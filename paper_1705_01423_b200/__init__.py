@@ -22,7 +22,8 @@ ERRORS = {-1: "AFID_ERR_NULL", -2: "AFID_ERR_ALIGN", -3: "AFID_ERR_UNSUPPORTED_S
 SYMBOLS = ["afid_plan_create", "afid_project", "afid_plan_destroy", "afid_plan_workspace_bytes",
            "afid_plan_num_launches", "afid_stage_forward", "afid_stage_solve", "afid_fft_length_supported",
            "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version",
-           "afid_plan_enable_timing", "afid_plan_kernel_times", "afid_plan_kernel_name"]
+           "afid_plan_enable_timing", "afid_plan_kernel_times", "afid_plan_kernel_name",
+           "afid_fft_half_length_supported"]
 
 _lib = None
 
@@ -58,6 +59,8 @@ def lib():
         L.afid_stage_solve.argtypes = [vp, vp, vp]
         L.afid_fft_length_supported.restype = i
         L.afid_fft_length_supported.argtypes = [i]
+        L.afid_fft_half_length_supported.restype = i
+        L.afid_fft_half_length_supported.argtypes = [i]
         L.afid_max_nx.restype = i
         L.afid_last_error.restype = C.c_char_p
         L.afid_last_error_code.restype = i
@@ -94,6 +97,10 @@ def _dev_ptr(t, n, name):
 
 def fft_length_supported(n):
     return bool(lib().afid_fft_length_supported(int(n)))
+
+
+def fft_half_length_supported(n):
+    return bool(lib().afid_fft_half_length_supported(int(n)))
 
 
 def max_nx():

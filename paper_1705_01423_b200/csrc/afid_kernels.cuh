@@ -39,6 +39,31 @@ struct DevParams {
 };
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
+// volatile read-only loads and a register "pin": see K1
+__device__ __forceinline__ double2 ldv2(const double* p)
+{
+    double2 r;
+    asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ double ldv1(const double* p)
+{
+    double r;
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(r) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void pin(double2& a) { asm volatile("" : "+d"(a.x), "+d"(a.y)); }
+__device__ __forceinline__ void pin1(double& a) { asm volatile("" : "+d"(a)); }
+__device__ __forceinline__ void l2_prefetch(const void* gptr, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gptr), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------
 // K1: divergence + r2c along z.  CTA = (i, group of NL consecutive j); NL*TPL threads.
@@ -47,19 +72,42 @@ __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterp
 // Output: B[i][jt][kz][jl] = spec_scale * X(kz), kz = 0..Nh.
 // ------------------------------------------------------------------------------------------
 template <class PL, int NL>
-__global__ void __launch_bounds__(NL* PL::TPL) k_div_r2c(DevParams P, const double* __restrict__ u,
+__global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_div_r2c(DevParams P, const double* __restrict__ u,
                                                          const double* __restrict__ v, const double* __restrict__ w,
-                                                         cplx* __restrict__ B)
+                                                         cplx* __restrict__ B, int pf_dist)
 {
     constexpr int Nh = PL::N, TPL = PL::TPL, LS = PL::LS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* sm = reinterpret_cast<cplx*>(smem_raw);
+    // CTA order: j-chunks of JC groups outermost, then i, then the group inside the chunk, so
+    // that plane i+1 of u (read again as plane i of the next step in i) is still in L2
     const int ngrp = P.ny / NL;
-    const int i = blockIdx.x / ngrp, jg = blockIdx.x % ngrp;
+    constexpr int JC = 64 / NL;
+    const int per_chunk = P.nx * JC;
+    int i, jg;
+    auto tile_of = [&](unsigned b, int& ti, int& tjg) {
+        const int chunk = b / per_chunk, rem = b % per_chunk;
+        const int jc_here = min(JC, ngrp - chunk * JC);
+        ti = rem / jc_here;
+        tjg = chunk * JC + rem % jc_here;
+    };
+    tile_of(blockIdx.x, i, jg);
+    const size_t plane = (size_t)P.ny * P.nz;
+    // L2 prefetch of the input lines of the CTA that starts about one CTA lifetime from now:
+    // ptxas keeps only 2-3 of this kernel's loads in flight per thread, which cannot cover DRAM
+    // latency; with the lines already in L2 it can.  One bulk prefetch per line.
+    if (pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x && threadIdx.x < 4 * NL + 1) {
+        int pi, pjg;
+        tile_of(blockIdx.x + pf_dist, pi, pjg);
+        const int a = threadIdx.x / NL, l = threadIdx.x % NL; // a: 0 u0, 1 u1, 2 v, 3 w, 4: v halo line
+        int pj = pjg * NL + l;
+        const double* base = (a <= 1) ? u + (size_t)(pi + a) * plane : (a == 3 ? w + (size_t)pi * plane : v + (size_t)pi * plane);
+        if (a == 4) pj = (pjg * NL + NL == P.ny) ? 0 : pjg * NL + NL;
+        l2_prefetch(base + (size_t)pj * P.nz, (unsigned)(P.nz * sizeof(double)));
+    }
     const int ln = threadIdx.x / TPL, tl = threadIdx.x % TPL;
     const int j = jg * NL + ln;
     const int jp = (j + 1 == P.ny) ? 0 : j + 1;
-    const size_t plane = (size_t)P.ny * P.nz;
     const double* u0 = u + (size_t)i * plane + (size_t)j * P.nz;
     const double* u1 = u0 + plane;
     const double* v0 = v + (size_t)i * plane + (size_t)j * P.nz;
@@ -68,22 +116,61 @@ __global__ void __launch_bounds__(NL* PL::TPL) k_div_r2c(DevParams P, const doub
     const double rdx = __ldg(&P.rdx[i]), rdy = P.rdy, rdz = P.rdz;
     cplx* line = sm + ln * LS;
 
-    // divergence of the two cells 2e, 2e+1 (P:L87 stencil)
-    auto ld_div = [&](int e) -> cplx {
-        const double2 a1 = ldg2(u1 + 2 * e), a0 = ldg2(u0 + 2 * e);
-        const double2 b1 = ldg2(v1 + 2 * e), b0 = ldg2(v0 + 2 * e);
-        const double2 c0 = ldg2(w0 + 2 * e);
-        const double cn = __ldg(w0 + ((e == Nh - 1) ? 0 : 2 * e + 2));
-        cplx d;
-        d.x = (a1.x - a0.x) * rdx + (b1.x - b0.x) * rdy + (c0.y - c0.x) * rdz;
-        d.y = (a1.y - a0.y) * rdx + (b1.y - b0.y) * rdy + (cn - c0.y) * rdz;
-        return d;
-    };
+    // divergence of the two cells 2e, 2e+1 (P:L87 stencil).  The loads are issued in batches
+    // of 2*NBATCH independent 16-byte loads (volatile PTX keeps them together; `pin` makes the
+    // arithmetic wait for the whole batch) -- otherwise ptxas interleaves each load with its
+    // consumer and the kernel is latency-bound at 2-3 loads in flight per thread.
     {
         typedef FftPass<PL, 0> P0;
+        constexpr int R = P0::R, NB = P0::NB;
+        constexpr int NBATCH = (R % 4 == 0) ? 4 : (R % 3 == 0 ? 3 : (R % 2 == 0 ? 2 : 1));
+        static_assert(P0::ROUNDS == 1, "K1 expects one first-pass butterfly per thread");
         typename P0::Regs rg;
-        P0::load(rg, tl, ld_div);
-        P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { line[PL::pad(e)] = val; });
+        const bool act = P0::EXACT || tl < NB;
+        if (act) {
+#pragma unroll
+            for (int h = 0; h < R; h += NBATCH) {
+                double2 x1[NBATCH], x0[NBATCH];
+#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2(u1 + 2 * (tl + NB * (h + r))); x0[r] = ldv2(u0 + 2 * (tl + NB * (h + r))); }
+#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) { pin(x1[r]); pin(x0[r]); }
+#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) rg.v[0][h + r] = mk((x1[r].x - x0[r].x) * rdx, (x1[r].y - x0[r].y) * rdx);
+            }
+#pragma unroll
+            for (int h = 0; h < R; h += NBATCH) {
+                double2 x1[NBATCH], x0[NBATCH];
+#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2(v1 + 2 * (tl + NB * (h + r))); x0[r] = ldv2(v0 + 2 * (tl + NB * (h + r))); }
+#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) { pin(x1[r]); pin(x0[r]); }
+#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) {
+                    rg.v[0][h + r].x = fma(x1[r].x - x0[r].x, rdy, rg.v[0][h + r].x);
+                    rg.v[0][h + r].y = fma(x1[r].y - x0[r].y, rdy, rg.v[0][h + r].y);
+                }
+            }
+#pragma unroll
+            for (int h = 0; h < R; h += NBATCH) {
+                double2 x0[NBATCH];
+                double cn[NBATCH];
+#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) {
+                    const int e = tl + NB * (h + r);
+                    x0[r] = ldv2(w0 + 2 * e);
+                    cn[r] = ldv1(w0 + ((e == Nh - 1) ? 0 : 2 * e + 2));
+                }
+#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) { pin(x0[r]); pin1(cn[r]); }
+#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) {
+                    rg.v[0][h + r].x = fma(x0[r].y - x0[r].x, rdz, rg.v[0][h + r].x);
+                    rg.v[0][h + r].y = fma(cn[r] - x0[r].y, rdz, rg.v[0][h + r].y);
+                }
+            }
+            P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { line[PL::pad(e)] = val; });
+        }
     }
     fft_tail_passes<PL, 1, true>(line, tl, true, P.tw_zh, [](int, cplx) {});
 
@@ -196,53 +283,65 @@ __global__ void __launch_bounds__(NL* tpl8<PL>()) k_ifft_y(DevParams P, const cp
 }
 
 // ------------------------------------------------------------------------------------------
-// K5: inverse c2r along z -> p.  CTA = (i, tile of 8 consecutive j); 8*TPL threads.
-// Gathers D[i][kz][8 j] (128-byte segments), forms Z'(k) = (X(k)+conj X(Nh-k)) + i conj(w^k)(X(k)-conj X(Nh-k)),
+// K5: inverse c2r along z -> p.  CTA = (i, tile of 8 consecutive j); LPR*TPL threads process the
+// 8 lines in 8/LPR rounds of LPR lines (registers hold one round; two CTAs per SM overlap one
+// CTA's gather with the other's transform).
+// Gathers D[i][kz][8 j] (128-byte segments, cp.async), forms in place
+//   Z'(k) = (X(k)+conj X(Nh-k)) + i conj(w^k)(X(k)-conj X(Nh-k)),
 // inverse complex FFT of length Nh gives z(m) = phi(2m) + i phi(2m+1).
 // ------------------------------------------------------------------------------------------
-template <class PL>
-__global__ void __launch_bounds__(8 * PL::TPL) k_c2r_z(DevParams P, const cplx* __restrict__ D, double* __restrict__ p)
+template <class PL, int LPR>
+__global__ void __launch_bounds__(LPR* PL::TPL) k_c2r_z(DevParams P, const cplx* __restrict__ D, double* __restrict__ p)
 {
-    constexpr int Nh = PL::N, TPL = PL::TPL, LS = PL::LS, NL = 8;
+    constexpr int Nh = PL::N, TPL = PL::TPL, LS = PL::LS, NL = 8, NT = LPR * TPL;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* sm = reinterpret_cast<cplx*>(smem_raw);
     const int njt = P.ny / 8;
     const int i = blockIdx.x / njt, jt = blockIdx.x % njt;
     const cplx* src = D + (size_t)i * P.nzh * (size_t)P.ny + (size_t)jt * 8;
-    for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NL * TPL) {
+    for (int idx = threadIdx.x; idx < (Nh + 1) * NL; idx += NT) {
+        const int k = idx >> 3, l = idx & 7;
+        cp_async16(&sm[l * LS + PL::pad(k)], &src[(size_t)k * P.ny + l]);
+    }
+    cp_async_wait_all();
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NT) {
         const int k = idx >> 3, l = idx & 7;
         const int km = Nh - k;
-        const cplx xk = __ldg(&src[(size_t)k * P.ny + l]);
-        const cplx xm = __ldg(&src[(size_t)km * P.ny + l]);
+        cplx* zl = sm + l * LS;
+        const cplx xk = zl[PL::pad(k)];
+        const cplx xm = zl[PL::pad(km)];
         const cplx wk = __ldg(&P.tw_z[k]);
         // E = X(k) + conj X(Nh-k), O = X(k) - conj X(Nh-k)
         const cplx E = mk(xk.x + xm.x, xk.y - xm.y), O = mk(xk.x - xm.x, xk.y + xm.y);
-        // i conj(w) O
         const cplx wo = mk(fma(wk.y, O.y, wk.x * O.x), fma(-wk.y, O.x, wk.x * O.y)); // conj(w) * O
-        const cplx t = mk(-wo.y, wo.x);
-        cplx* zl = sm + l * LS;
+        const cplx t = mk(-wo.y, wo.x);                                              // i conj(w) O
         // stored re/im-swapped: the inverse transform runs as a forward one on swapped data
         zl[PL::pad(k)] = mk(E.y + t.y, E.x + t.x);
-        // Z'(Nh-k) = conj(E) + i conj(w^(Nh-k)) (-conj O) = conj(E) + i w^k ... = conj( E - i conj(w) O )
+        // Z'(Nh-k) = conj( E - i conj(w) O )
         if (k != 0 && k != km) zl[PL::pad(km)] = mk(-(E.y - t.y), E.x - t.x);
     }
     __syncthreads();
-    const int ln = threadIdx.x / TPL, tl = threadIdx.x % TPL;
-    cplx* line = sm + ln * LS;
-    double* dst = p + ((size_t)i * P.ny + (size_t)jt * 8 + ln) * (size_t)P.nz;
-    auto st_p = [&](int e, cplx val) { reinterpret_cast<double2*>(dst)[e] = cswap(val); };
-    typedef FftPass<PL, 0> P0;
-    {
-        typename P0::Regs rg;
-        P0::load(rg, tl, [&](int e) { return line[PL::pad(e)]; });
-        if constexpr (PL::NPASS == 1) {
-            P0::compute_store(rg, tl, P.tw_zh, st_p);
-        } else {
-            __syncthreads();
-            P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { line[PL::pad(e)] = val; });
+    const int lr = threadIdx.x / TPL, tl = threadIdx.x % TPL;
+#pragma unroll 1
+    for (int rnd = 0; rnd < NL / LPR; ++rnd) {
+        const int ln = rnd * LPR + lr;
+        cplx* line = sm + ln * LS;
+        double* dst = p + ((size_t)i * P.ny + (size_t)jt * 8 + ln) * (size_t)P.nz;
+        auto st_p = [&](int e, cplx val) { reinterpret_cast<double2*>(dst)[e] = cswap(val); };
+        typedef FftPass<PL, 0> P0;
+        {
+            typename P0::Regs rg;
+            P0::load(rg, tl, [&](int e) { return line[PL::pad(e)]; });
+            if constexpr (PL::NPASS == 1) {
+                P0::compute_store(rg, tl, P.tw_zh, st_p);
+            } else {
+                __syncthreads();
+                P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { line[PL::pad(e)] = val; });
+            }
         }
+        if constexpr (PL::NPASS > 1) fft_tail_passes<PL, 1, false>(line, tl, true, P.tw_zh, st_p);
     }
-    if constexpr (PL::NPASS > 1) fft_tail_passes<PL, 1, false>(line, tl, true, P.tw_zh, st_p);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -252,13 +351,23 @@ __global__ void __launch_bounds__(8 * PL::TPL) k_c2r_z(DevParams P, const cplx* 
 __global__ void __launch_bounds__(256) k_correct(DevParams P, const double* __restrict__ p, double* __restrict__ u,
                                                  double* __restrict__ v, double* __restrict__ w)
 {
+    // work order: j-chunks of JC lines outermost, then i, then the line inside the chunk, so that
+    // plane i-1 of p (read again for the x-gradient) is still in L2 when plane i is processed
     const int nzh2 = P.nz / 2;
+    constexpr int JC = 32;
     const size_t npair = (size_t)P.nx * P.ny * nzh2;
     const size_t plane = (size_t)P.ny * P.nz;
+    const size_t chunk_pairs = (size_t)P.nx * JC * nzh2;
     for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < npair; t += (size_t)gridDim.x * blockDim.x) {
-        const int kp = (int)(t % nzh2);
-        const size_t ij = t / nzh2;
-        const int j = (int)(ij % P.ny), i = (int)(ij / P.ny);
+        const int chunk = (int)(t / chunk_pairs);
+        const size_t rem = t % chunk_pairs;
+        const int jc_here = min(JC, P.ny - chunk * JC);
+        const size_t slab = (size_t)jc_here * nzh2;
+        const int i = (int)(rem / slab);
+        const size_t r2 = rem % slab;
+        const int j = chunk * JC + (int)(r2 / nzh2);
+        const int kp = (int)(r2 % nzh2);
+        const size_t ij = (size_t)i * P.ny + j;
         const size_t o = ij * P.nz + 2 * (size_t)kp;
         const double2 ph = ldg2(p + o);
         const size_t ojm = (j == 0) ? o + (size_t)(P.ny - 1) * P.nz : o - P.nz;
@@ -314,12 +423,6 @@ __device__ __forceinline__ double fast_rcp(double x)
     return r;
 }
 
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
-{
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 template <int M>
 __global__ void __launch_bounds__(M == 4 ? 128 : (M == 16 ? 512 : 384)) k_solve_x(DevParams P, const cplx* __restrict__ C, cplx* __restrict__ T)

@@ -49,46 +49,79 @@ int fail(int code, const std::string& msg)
     X(3072, 16, 16, 12, 1, 192) \
     X(4096, 16, 16, 16, 1, 256)
 
+// z-direction lines (K1, K5; complex length nz/2): plans with <= 12 elements per thread where
+// it matters, so that twice as many warps are resident while the loads are in flight
+#define AFID_FFT_SIZES_Z(X)     \
+    X(8, 8, 1, 1, 1, 1)         \
+    X(16, 16, 1, 1, 1, 1)       \
+    X(24, 8, 3, 1, 1, 3)        \
+    X(32, 8, 4, 1, 1, 4)        \
+    X(48, 16, 3, 1, 1, 4)       \
+    X(64, 8, 8, 1, 1, 8)        \
+    X(96, 16, 6, 1, 1, 8)       \
+    X(128, 16, 8, 1, 1, 8)      \
+    X(192, 16, 12, 1, 1, 16)    \
+    X(256, 16, 16, 1, 1, 16)    \
+    X(384, 8, 8, 6, 1, 48)      \
+    X(512, 8, 8, 8, 1, 64)      \
+    X(768, 16, 16, 3, 1, 48)    \
+    X(1024, 8, 16, 8, 1, 128)
+
 constexpr int K1_NL = 4; // lines per CTA in K1 (two CTAs fill one 128-byte row of B)
+constexpr int K5_LPR = 4; // lines per round in K5 (8 lines per CTA, 2 rounds)
 constexpr int KY_NL = 2; // lines per CTA in K2 / K4 (256-byte gather segments)
-constexpr int MAX_ZH = 1024; // largest nz/2 for which K5's 8-line tile fits shared memory
 
 struct LaunchCfg {
     const void* fn;
     int threads;
     size_t smem;
+    int ctas_per_sm; // CTAs per SM the shared-memory carveout is sized for (the rest stays L1)
 };
 
 template <class PL> LaunchCfg cfg_k1()
 {
-    return {(const void*)k_div_r2c<PL, K1_NL>, K1_NL * PL::TPL, (size_t)K1_NL * PL::LS * sizeof(cplx)};
+    return {(const void*)k_div_r2c<PL, K1_NL>, K1_NL * PL::TPL, (size_t)K1_NL * PL::LS * sizeof(cplx), 3};
 }
 template <class PL> LaunchCfg cfg_k2()
 {
-    return {(const void*)k_fft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx)};
+    return {(const void*)k_fft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx), 3};
 }
 template <class PL> LaunchCfg cfg_k4()
 {
-    return {(const void*)k_ifft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx)};
+    return {(const void*)k_ifft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx), 3};
 }
 template <class PL> LaunchCfg cfg_k5()
 {
-    return {(const void*)k_c2r_z<PL>, 8 * PL::TPL, (size_t)8 * PL::LS * sizeof(cplx)};
+    return {(const void*)k_c2r_z<PL, K5_LPR>, K5_LPR * PL::TPL, (size_t)8 * PL::LS * sizeof(cplx), 2};
 }
 
-bool lookup_fft(int n, LaunchCfg* k1, LaunchCfg* k2, LaunchCfg* k4, LaunchCfg* k5)
+bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4)
+{
+    switch (n) {
+#define X(N, R0, R1, R2, R3, TPL)                   \
+    case N: {                                       \
+        typedef FftPlan<R0, R1, R2, R3, TPL> PL;    \
+        if (k2) *k2 = cfg_k2<PL>();                 \
+        if (k4) *k4 = cfg_k4<PL>();                 \
+        return true;                                \
+    }
+        AFID_FFT_SIZES(X)
+#undef X
+    default:
+        return false;
+    }
+}
+bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5)
 {
     switch (n) {
 #define X(N, R0, R1, R2, R3, TPL)                   \
     case N: {                                       \
         typedef FftPlan<R0, R1, R2, R3, TPL> PL;    \
         if (k1) *k1 = cfg_k1<PL>();                 \
-        if (k2) *k2 = cfg_k2<PL>();                 \
-        if (k4) *k4 = cfg_k4<PL>();                 \
         if (k5) *k5 = cfg_k5<PL>();                 \
         return true;                                \
     }
-        AFID_FFT_SIZES(X)
+        AFID_FFT_SIZES_Z(X)
 #undef X
     default:
         return false;
@@ -108,6 +141,7 @@ struct afid_plan {
     size_t ws_bytes;
     LaunchCfg k1, k2, k4, k5, k3;
     int n_sm;
+    int k1_pf;         // K1's L2-prefetch distance in CTAs
     // optional per-kernel timing (afid_plan_enable_timing): NK+1 events around the NK kernels
     bool timing;
     cudaEvent_t ev[7];
@@ -122,10 +156,20 @@ const char* afid_version(void) { return "afid-project-b200 0.1 (sm_100a, fp64)";
 const char* afid_last_error(void) { return g_err.c_str(); }
 int afid_last_error_code(void) { return g_err_code; }
 int afid_max_nx(void) { return MAX_NX; }
-int afid_fft_length_supported(int n) { return lookup_fft(n, nullptr, nullptr, nullptr, nullptr) ? 1 : 0; }
+int afid_fft_length_supported(int n) { return lookup_fft_y(n, nullptr, nullptr) ? 1 : 0; }
+int afid_fft_half_length_supported(int n) { return lookup_fft_z(n, nullptr, nullptr) ? 1 : 0; }
 
 static int set_smem_attr(const LaunchCfg& c)
 {
+    // ask for the largest shared-memory carveout so that several CTAs fit per SM
+    {
+        const size_t per_sm = 228 * 1024;
+        size_t want = (size_t)c.ctas_per_sm * (c.smem + 1024);
+        if (want > per_sm) want = per_sm;
+        int pct = (int)((want * 100 + per_sm - 1) / per_sm);
+        if (getenv("AFID_CARVEOUT")) pct = atoi(getenv("AFID_CARVEOUT"));
+        if (pct >= 0) cudaFuncSetAttribute(c.fn, cudaFuncAttributePreferredSharedMemoryCarveout, pct);
+    }
     if (c.smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(c.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
         if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
@@ -147,8 +191,8 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     afid_plan* pl = new (std::nothrow) afid_plan();
     if (!pl) { fail(AFID_ERR_NOMEM, "host allocation failed"); return nullptr; }
     std::memset(pl, 0, sizeof(*pl));
-    if (!lookup_fft(ny, nullptr, &pl->k2, &pl->k4, nullptr)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "ny is not a supported FFT length"); return nullptr; }
-    if (nh > MAX_ZH || !lookup_fft(nh, &pl->k1, nullptr, nullptr, &pl->k5)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "nz/2 is not a supported FFT length"); return nullptr; }
+    if (!lookup_fft_y(ny, &pl->k2, &pl->k4)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "ny is not a supported FFT length"); return nullptr; }
+    if (!lookup_fft_z(nh, &pl->k1, &pl->k5)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "nz/2 is not a supported FFT length"); return nullptr; }
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
 
     // ---- K3 configuration
@@ -159,6 +203,7 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     pch = (nx + M - 1) / M;
     pl->k3.threads = 8 * pch;
     pl->k3.smem = (size_t)nx * 8 * sizeof(cplx) + (size_t)10 * pch * 8 * sizeof(double);
+    pl->k3.ctas_per_sm = 4;
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -167,6 +212,7 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     }
     if (prop.major != 10) { delete pl; fail(AFID_ERR_CUDA, "this library is built for sm_100a (B200) only"); return nullptr; }
     pl->n_sm = prop.multiProcessorCount;
+    pl->k1_pf = getenv("AFID_K1_PF") ? atoi(getenv("AFID_K1_PF")) : 4 * pl->n_sm;
     for (const LaunchCfg* c : {&pl->k1, &pl->k2, &pl->k3, &pl->k4, &pl->k5}) {
         if (c->smem > prop.sharedMemPerBlockOptin) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "tile does not fit shared memory"); return nullptr; }
         if (set_smem_attr(*c) != AFID_OK) { delete pl; return nullptr; }
@@ -279,7 +325,8 @@ static int run_forward(afid_plan* pl, const double* u, const double* v, const do
 {
     int rc;
     {
-        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB};
+        int pf = pl->k1_pf;
+        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &pf};
         rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c");
         if (rc) return rc;
     }
@@ -307,7 +354,8 @@ int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void
     cplx* wsC = pl->ws[1];
     if (tm) cudaEventRecord(pl->ev[0], st);
     {
-        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB};   // B in ws0
+        int pf = pl->k1_pf;
+        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &pf};   // B in ws0
         if ((rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c"))) return rc;
     }
     if (tm) cudaEventRecord(pl->ev[1], st);
@@ -329,7 +377,7 @@ int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void
     }
     if (tm) cudaEventRecord(pl->ev[5], st);
     {
-        LaunchCfg c = {(const void*)k_correct, 256, 0};
+        LaunchCfg c = {(const void*)k_correct, 256, 0, 0};
         void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w};
         const size_t npair = (size_t)pl->nx * pl->ny * (pl->nz / 2);
         size_t blocks = (npair + 255) / 256;

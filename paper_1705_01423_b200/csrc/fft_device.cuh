@@ -154,8 +154,8 @@ template <int R0_, int R1_, int R2_, int R3_, int TPL_> struct FftPlan {
     // Shared-memory layout of a line: one pad element after every R0 elements, so that the
     // first pass's stride-R0 writes are bank-conflict free; line stride odd (in 16-byte
     // units) so that 8 lines accessed at the same offset hit 8 different bank groups.
-    static constexpr int PADDED = N + N / R0;
-    static constexpr int LS = (PADDED % 2 == 0) ? PADDED + 1 : PADDED;
+    static constexpr int PADDED = N + N / R0; // = pad(N): one extra slot (index N) is kept for K5's Nyquist entry
+    static constexpr int LS = (PADDED % 2 == 0) ? PADDED + 1 : PADDED + 2;
     static __device__ __forceinline__ int pad(int e) { return e + e / R0; }
     template <int P> static constexpr int radix() { return P == 0 ? R0 : (P == 1 ? R1 : (P == 2 ? R2 : R3)); }
     template <int P> static constexpr int stride() { return P == 0 ? 1 : (P == 1 ? R0 : (P == 2 ? R0 * R1 : R0 * R1 * R2)); }
@@ -198,8 +198,21 @@ template <class PL, int P> struct FftPass {
                 const int t = b % S, q = b / S;
                 if (M > 1) {
                     const int e = q * S;
+                    if (S == 1) {
+                        // first pass: every butterfly has its own twiddle base w = tw[b]; one
+                        // coalesced load, the powers w^r by a depth-log2(r) product tree
+                        // (a gather of tw[b*r] would touch up to 32 cache lines per warp load)
+                        cplx wp[R];
+                        wp[1] = __ldg(&tw[e]);
 #pragma unroll
-                    for (int r = 1; r < R; ++r) rg.v[rd][r] = cmul(rg.v[rd][r], __ldg(&tw[e * r]));
+                        for (int r = 2; r < R; ++r) wp[r] = cmul(wp[r / 2], wp[r - r / 2]);
+#pragma unroll
+                        for (int r = 1; r < R; ++r) rg.v[rd][r] = cmul(rg.v[rd][r], wp[r]);
+                    } else {
+                        // later passes: S consecutive butterflies share q, the loads are broadcasts
+#pragma unroll
+                        for (int r = 1; r < R; ++r) rg.v[rd][r] = cmul(rg.v[rd][r], __ldg(&tw[e * r]));
+                    }
                 }
                 const int o = t + S * R * q;
 #pragma unroll
