@@ -52,12 +52,9 @@ __device__ __forceinline__ double ldv1(const double* p)
     asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(r) : "l"(p));
     return r;
 }
+#define SCHED_FENCE() __syncwarp()
 __device__ __forceinline__ void pin(double2& a) { asm volatile("" : "+d"(a.x), "+d"(a.y)); }
 __device__ __forceinline__ void pin1(double& a) { asm volatile("" : "+d"(a)); }
-__device__ __forceinline__ void l2_prefetch(const void* gptr, unsigned bytes)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gptr), "r"(bytes) : "memory");
-}
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
 {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -74,7 +71,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 template <class PL, int NL>
 __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_div_r2c(DevParams P, const double* __restrict__ u,
                                                          const double* __restrict__ v, const double* __restrict__ w,
-                                                         cplx* __restrict__ B, int pf_dist)
+                                                         cplx* __restrict__ B, int i_base, int np, int bmod)
 {
     constexpr int Nh = PL::N, TPL = PL::TPL, LS = PL::LS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -83,28 +80,16 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
     // that plane i+1 of u (read again as plane i of the next step in i) is still in L2
     const int ngrp = P.ny / NL;
     constexpr int JC = 64 / NL;
-    const int per_chunk = P.nx * JC;
+    // this launch covers planes i_base .. i_base+np-1
+    const int per_chunk = np * JC;
     int i, jg;
-    auto tile_of = [&](unsigned b, int& ti, int& tjg) {
-        const int chunk = b / per_chunk, rem = b % per_chunk;
+    {
+        const int chunk = blockIdx.x / per_chunk, rem = blockIdx.x % per_chunk;
         const int jc_here = min(JC, ngrp - chunk * JC);
-        ti = rem / jc_here;
-        tjg = chunk * JC + rem % jc_here;
-    };
-    tile_of(blockIdx.x, i, jg);
-    const size_t plane = (size_t)P.ny * P.nz;
-    // L2 prefetch of the input lines of the CTA that starts about one CTA lifetime from now:
-    // ptxas keeps only 2-3 of this kernel's loads in flight per thread, which cannot cover DRAM
-    // latency; with the lines already in L2 it can.  One bulk prefetch per line.
-    if (pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x && threadIdx.x < 4 * NL + 1) {
-        int pi, pjg;
-        tile_of(blockIdx.x + pf_dist, pi, pjg);
-        const int a = threadIdx.x / NL, l = threadIdx.x % NL; // a: 0 u0, 1 u1, 2 v, 3 w, 4: v halo line
-        int pj = pjg * NL + l;
-        const double* base = (a <= 1) ? u + (size_t)(pi + a) * plane : (a == 3 ? w + (size_t)pi * plane : v + (size_t)pi * plane);
-        if (a == 4) pj = (pjg * NL + NL == P.ny) ? 0 : pjg * NL + NL;
-        l2_prefetch(base + (size_t)pj * P.nz, (unsigned)(P.nz * sizeof(double)));
+        i = i_base + rem / jc_here;
+        jg = chunk * JC + rem % jc_here;
     }
+    const size_t plane = (size_t)P.ny * P.nz;
     const int ln = threadIdx.x / TPL, tl = threadIdx.x % TPL;
     const int j = jg * NL + ln;
     const int jp = (j + 1 == P.ny) ? 0 : j + 1;
@@ -134,6 +119,7 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2(u1 + 2 * (tl + NB * (h + r))); x0[r] = ldv2(u0 + 2 * (tl + NB * (h + r))); }
 #pragma unroll
+                SCHED_FENCE();
                 for (int r = 0; r < NBATCH; ++r) { pin(x1[r]); pin(x0[r]); }
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) rg.v[0][h + r] = mk((x1[r].x - x0[r].x) * rdx, (x1[r].y - x0[r].y) * rdx);
@@ -144,6 +130,7 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2(v1 + 2 * (tl + NB * (h + r))); x0[r] = ldv2(v0 + 2 * (tl + NB * (h + r))); }
 #pragma unroll
+                SCHED_FENCE();
                 for (int r = 0; r < NBATCH; ++r) { pin(x1[r]); pin(x0[r]); }
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) {
@@ -162,6 +149,7 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
                     cn[r] = ldv1(w0 + ((e == Nh - 1) ? 0 : 2 * e + 2));
                 }
 #pragma unroll
+                SCHED_FENCE();
                 for (int r = 0; r < NBATCH; ++r) { pin(x0[r]); pin1(cn[r]); }
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) {
@@ -176,7 +164,8 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
 
     // split into the spectrum of the real line; thread -> (k, jl) with jl fastest
     const int jl0 = (jg * NL) % 8;         // position of this CTA's first line inside the tile
-    cplx* out = B + ((size_t)i * (P.ny / 8) + (size_t)(jg * NL / 8)) * (size_t)P.nzh * 8;
+    // B may be a rotating buffer of bmod planes (plane-batched launches keep it L2-resident)
+    cplx* out = B + ((size_t)(i % bmod) * (P.ny / 8) + (size_t)(jg * NL / 8)) * (size_t)P.nzh * 8;
     const double hs = 0.5 * P.spec_scale;
     for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NL * TPL) {
         const int k = idx / NL, l = idx % NL;
@@ -206,20 +195,20 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
 template <class PL> constexpr int tpl8() { return (PL::TPL + 7) / 8 * 8; }
 
 template <class PL, int NL>
-__global__ void __launch_bounds__(NL* tpl8<PL>()) k_fft_y(DevParams P, const cplx* __restrict__ B, cplx* __restrict__ C)
+__global__ void __launch_bounds__(NL* tpl8<PL>()) k_fft_y(DevParams P, const cplx* __restrict__ B, cplx* __restrict__ C, int i_base, int bmod)
 {
     constexpr int TPL = PL::TPL, LS = PL::LS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* sm = reinterpret_cast<cplx*>(smem_raw);
     const int ngrp = (P.nzh + NL - 1) / NL;
-    const int i = blockIdx.x / ngrp, kg = blockIdx.x % ngrp;
+    const int i = i_base + blockIdx.x / ngrp, kg = blockIdx.x % ngrp;
     // interleave the NL lines at 8-thread granularity so that a warp's loads cover
     // NL*128 contiguous bytes of B
     const int ln = (threadIdx.x >> 3) % NL;
     const int tl = (threadIdx.x & 7) | ((threadIdx.x / (8 * NL)) << 3);
     const int kz = kg * NL + ln;
     const bool active = (kz < P.nzh) && (tl < TPL);
-    const cplx* src = B + (size_t)i * (P.ny / 8) * (size_t)P.nzh * 8 + (size_t)kz * 8;
+    const cplx* src = B + (size_t)(i % bmod) * (P.ny / 8) * (size_t)P.nzh * 8 + (size_t)kz * 8;
     const size_t tile_stride = (size_t)P.nzh * 8;
     cplx* dst = C + ((size_t)i * P.nzh + kz) * (size_t)P.ny;
     cplx* line = sm + ln * LS;

@@ -141,7 +141,11 @@ struct afid_plan {
     size_t ws_bytes;
     LaunchCfg k1, k2, k4, k5, k3;
     int n_sm;
-    int k1_pf;         // K1's L2-prefetch distance in CTAs
+    // plane-batched forward sweep (K1 -> K2 through an L2-resident rotating B buffer)
+    int s1_batch;      // planes per batch; 0 = one launch for all planes
+    int s1_nstreams;
+    cudaStream_t aux[8];
+    cudaEvent_t ev_fork, ev_join[8];
     // optional per-kernel timing (afid_plan_enable_timing): NK+1 events around the NK kernels
     bool timing;
     cudaEvent_t ev[7];
@@ -212,7 +216,17 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     }
     if (prop.major != 10) { delete pl; fail(AFID_ERR_CUDA, "this library is built for sm_100a (B200) only"); return nullptr; }
     pl->n_sm = prop.multiProcessorCount;
-    pl->k1_pf = getenv("AFID_K1_PF") ? atoi(getenv("AFID_K1_PF")) : 4 * pl->n_sm;
+    pl->s1_batch = getenv("AFID_S1_BATCH") ? atoi(getenv("AFID_S1_BATCH")) : 0;
+    pl->s1_nstreams = getenv("AFID_S1_STREAMS") ? atoi(getenv("AFID_S1_STREAMS")) : 3;
+    if (pl->s1_nstreams < 1) pl->s1_nstreams = 1;
+    if (pl->s1_nstreams > 8) pl->s1_nstreams = 8;
+    if (pl->s1_batch > 0) {
+        cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming);
+        for (int k = 0; k < pl->s1_nstreams; ++k) {
+            cudaStreamCreateWithFlags(&pl->aux[k], cudaStreamNonBlocking);
+            cudaEventCreateWithFlags(&pl->ev_join[k], cudaEventDisableTiming);
+        }
+    }
     for (const LaunchCfg* c : {&pl->k1, &pl->k2, &pl->k3, &pl->k4, &pl->k5}) {
         if (c->smem > prop.sharedMemPerBlockOptin) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "tile does not fit shared memory"); return nullptr; }
         if (set_smem_attr(*c) != AFID_OK) { delete pl; return nullptr; }
@@ -321,20 +335,51 @@ static int check_ptr(const void* p, const char* name)
 }
 
 // K1 + K2: u,v,w -> C layout spectrum in `outC`
-static int run_forward(afid_plan* pl, const double* u, const double* v, const double* w, cplx* wsB, cplx* outC, cudaStream_t st)
+static int run_forward(afid_plan* pl, const double* u, const double* v, const double* w, cplx* wsB, cplx* outC, cudaStream_t st,
+                       cudaEvent_t ev_mid)
 {
     int rc;
-    {
-        int pf = pl->k1_pf;
-        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &pf};
-        rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c");
-        if (rc) return rc;
+    const int ngrp2 = (pl->nzh + KY_NL - 1) / KY_NL;
+    if (pl->s1_batch <= 0) {
+        int i_base = 0, np = pl->nx, bmod = pl->nx;
+        {
+            void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &i_base, &np, &bmod};
+            rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c");
+            if (rc) return rc;
+        }
+        if (ev_mid) cudaEventRecord(ev_mid, st);
+        {
+            void* args[] = {&pl->dp, (void*)&wsB, (void*)&outC, &i_base, &bmod};
+            rc = launch(pl->k2, (unsigned)(pl->nx * ngrp2), st, args, "k_fft_y");
+        }
+        return rc;
     }
-    {
-        void* args[] = {&pl->dp, (void*)&wsB, (void*)&outC};
-        rc = launch(pl->k2, (unsigned)(pl->nx * ((pl->nzh + KY_NL - 1) / KY_NL)), st, args, "k_fft_y");
+    // plane-batched: batch k runs K1 then K2 on aux stream k % ns, B slot = stream index
+    const int nb = pl->s1_batch, ns = pl->s1_nstreams;
+    int bmod = nb * ns;
+    cudaEventRecord(pl->ev_fork, st);
+    for (int k = 0; k < ns; ++k) cudaStreamWaitEvent(pl->aux[k], pl->ev_fork, 0);
+    int kb = 0;
+    for (int i_base = 0; i_base < pl->nx; i_base += nb, ++kb) {
+        int np = (pl->nx - i_base < nb) ? pl->nx - i_base : nb;
+        cudaStream_t s = pl->aux[kb % ns];
+        {
+            void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &i_base, &np, &bmod};
+            rc = launch(pl->k1, (unsigned)(np * (pl->ny / K1_NL)), s, args, "k_div_r2c");
+            if (rc) return rc;
+        }
+        {
+            void* args[] = {&pl->dp, (void*)&wsB, (void*)&outC, &i_base, &bmod};
+            rc = launch(pl->k2, (unsigned)(np * ngrp2), s, args, "k_fft_y");
+            if (rc) return rc;
+        }
     }
-    return rc;
+    for (int k = 0; k < ns; ++k) {
+        cudaEventRecord(pl->ev_join[k], pl->aux[k]);
+        cudaStreamWaitEvent(st, pl->ev_join[k], 0);
+    }
+    if (ev_mid) cudaEventRecord(ev_mid, st);
+    return AFID_OK;
 }
 
 static int run_solve(afid_plan* pl, const cplx* inC, cplx* outT, cudaStream_t st)
@@ -353,16 +398,7 @@ int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void
     cplx* wsB = pl->ws[0];
     cplx* wsC = pl->ws[1];
     if (tm) cudaEventRecord(pl->ev[0], st);
-    {
-        int pf = pl->k1_pf;
-        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &pf};   // B in ws0
-        if ((rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c"))) return rc;
-    }
-    if (tm) cudaEventRecord(pl->ev[1], st);
-    {
-        void* args[] = {&pl->dp, (void*)&wsB, (void*)&wsC};                        // C in ws1
-        if ((rc = launch(pl->k2, (unsigned)(pl->nx * ((pl->nzh + KY_NL - 1) / KY_NL)), st, args, "k_fft_y"))) return rc;
-    }
+    if ((rc = run_forward(pl, u, v, w, wsB, wsC, st, tm ? pl->ev[1] : nullptr))) return rc;   // B in ws0, C in ws1
     if (tm) cudaEventRecord(pl->ev[2], st);
     if ((rc = run_solve(pl, pl->ws[1], pl->ws[0], st))) return rc;             // T in ws0
     if (tm) cudaEventRecord(pl->ev[3], st);
@@ -426,7 +462,7 @@ int afid_stage_forward(afid_plan* pl, const double* u, const double* v, const do
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     int rc;
     if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(spec, "spec"))) return rc;
-    return run_forward(pl, u, v, w, pl->ws[0], (cplx*)spec, (cudaStream_t)stream);
+    return run_forward(pl, u, v, w, pl->ws[0], (cplx*)spec, (cudaStream_t)stream, nullptr);
 }
 
 // in place on a C-layout array: K3 writes the T layout into ws0, then a re-layout kernel is
