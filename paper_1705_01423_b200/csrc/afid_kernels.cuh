@@ -36,7 +36,41 @@ struct DevParams {
     const cplx* tw_zh;          // [nz/2]  exp(-2 pi i k/(nz/2))
     const cplx* tw_z;           // [nz/2+1] exp(-2 pi i k/nz)
     double inv_vol;             // 1/sum dx_i
+    int hints;                  // L2 eviction-priority switches (bit mask, see l2_policy users)
 };
+
+// L2 eviction priorities (PTX createpolicy): 0 = normal, 1 = evict_first (streamed once), 2 = evict_last (kept)
+__device__ __forceinline__ unsigned long long l2_policy(int kind)
+{
+    unsigned long long p;
+    if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    else if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ double2 ldv2h(const double* p, unsigned long long pol)
+{
+    double2 r;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ double ldv1h(const double* p, unsigned long long pol)
+{
+    double r;
+    asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(r) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ cplx ldc_h(const cplx* p, unsigned long long pol)
+{
+    cplx r;
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ void stc_h(cplx* p, cplx v, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void l2_discard128(const void* p) { asm volatile("discard.global.L2 [%0], 128;" ::"l"(p) : "memory"); }
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
 // volatile read-only loads and a register "pin": see K1
@@ -52,13 +86,20 @@ __device__ __forceinline__ double ldv1(const double* p)
     asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(r) : "l"(p));
     return r;
 }
-#define SCHED_FENCE() __syncwarp()
+// scheduling fence between a load batch and its consumers; only the converged lanes take part
+// (the callers sit inside `if (act)`: a full-mask __syncwarp there would hang on partial warps)
+#define SCHED_FENCE() __syncwarp(__activemask())
 __device__ __forceinline__ void pin(double2& a) { asm volatile("" : "+d"(a.x), "+d"(a.y)); }
 __device__ __forceinline__ void pin1(double& a) { asm volatile("" : "+d"(a)); }
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
 {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async16h(void* smem_dst, const void* gsrc, unsigned long long pol)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
@@ -100,6 +141,8 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
     const double* w0 = w + (size_t)i * plane + (size_t)j * P.nz;
     const double rdx = __ldg(&P.rdx[i]), rdy = P.rdy, rdz = P.rdz;
     cplx* line = sm + ln * LS;
+    const unsigned long long pol_in = l2_policy((P.hints & 1) ? 1 : 0), pol_u1 = l2_policy(0);
+    const unsigned long long pol_b = l2_policy((P.hints & 2) ? 2 : 0);
 
     // divergence of the two cells 2e, 2e+1 (P:L87 stencil).  The loads are issued in batches
     // of 2*NBATCH independent 16-byte loads (volatile PTX keeps them together; `pin` makes the
@@ -117,9 +160,9 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
             for (int h = 0; h < R; h += NBATCH) {
                 double2 x1[NBATCH], x0[NBATCH];
 #pragma unroll
-                for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2(u1 + 2 * (tl + NB * (h + r))); x0[r] = ldv2(u0 + 2 * (tl + NB * (h + r))); }
-#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2h(u1 + 2 * (tl + NB * (h + r)), pol_u1); x0[r] = ldv2h(u0 + 2 * (tl + NB * (h + r)), pol_in); }
                 SCHED_FENCE();
+#pragma unroll
                 for (int r = 0; r < NBATCH; ++r) { pin(x1[r]); pin(x0[r]); }
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) rg.v[0][h + r] = mk((x1[r].x - x0[r].x) * rdx, (x1[r].y - x0[r].y) * rdx);
@@ -128,9 +171,9 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
             for (int h = 0; h < R; h += NBATCH) {
                 double2 x1[NBATCH], x0[NBATCH];
 #pragma unroll
-                for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2(v1 + 2 * (tl + NB * (h + r))); x0[r] = ldv2(v0 + 2 * (tl + NB * (h + r))); }
-#pragma unroll
+                for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2h(v1 + 2 * (tl + NB * (h + r)), pol_u1); x0[r] = ldv2h(v0 + 2 * (tl + NB * (h + r)), pol_in); }
                 SCHED_FENCE();
+#pragma unroll
                 for (int r = 0; r < NBATCH; ++r) { pin(x1[r]); pin(x0[r]); }
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) {
@@ -145,11 +188,11 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) {
                     const int e = tl + NB * (h + r);
-                    x0[r] = ldv2(w0 + 2 * e);
-                    cn[r] = ldv1(w0 + ((e == Nh - 1) ? 0 : 2 * e + 2));
+                    x0[r] = ldv2h(w0 + 2 * e, pol_in);
+                    cn[r] = ldv1h(w0 + ((e == Nh - 1) ? 0 : 2 * e + 2), pol_in);
                 }
-#pragma unroll
                 SCHED_FENCE();
+#pragma unroll
                 for (int r = 0; r < NBATCH; ++r) { pin(x0[r]); pin1(cn[r]); }
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) {
@@ -183,8 +226,8 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
         // Z(Nh-k) + conj Z(k) = conj(E);  Z(Nh-k) - conj Z(k) = -conj(O);  w^(Nh-k) = -conj(w^k)
         // X(Nh-k) = 1/2 [ conj(E) - i (-conj w)(-conj O) ] = 1/2 [ conj(E) - i conj(w O) ] = 1/2 conj( E + i w O )
         const cplx xm = mk(hs * (E.x - t.x), -hs * (E.y - t.y));
-        out[(size_t)k * 8 + jl0 + l] = xk;
-        if (k != Nh - k) out[(size_t)(Nh - k) * 8 + jl0 + l] = xm;
+        stc_h(&out[(size_t)k * 8 + jl0 + l], xk, pol_b);
+        if (k != Nh - k) stc_h(&out[(size_t)(Nh - k) * 8 + jl0 + l], xm, pol_b);
     }
 }
 
@@ -212,8 +255,16 @@ __global__ void __launch_bounds__(NL* tpl8<PL>()) k_fft_y(DevParams P, const cpl
     const size_t tile_stride = (size_t)P.nzh * 8;
     cplx* dst = C + ((size_t)i * P.nzh + kz) * (size_t)P.ny;
     cplx* line = sm + ln * LS;
-    auto ld_b = [&](int e) -> cplx { return __ldg(&src[(size_t)(e >> 3) * tile_stride + (e & 7)]); };
-    auto st_c = [&](int e, cplx val) { dst[e] = val; };
+    const unsigned long long pol_b = l2_policy((P.hints & 4) ? 1 : ((P.hints & 2) ? 2 : 0));
+    const unsigned long long pol_c = l2_policy((P.hints & 8) ? 1 : 0);
+    const bool discard_b = (P.hints & 16) != 0;
+    auto ld_b = [&](int e) -> cplx {
+        const cplx* a = &src[(size_t)(e >> 3) * tile_stride + (e & 7)];
+        const cplx r = ldc_h(a, pol_b);
+        if (discard_b && (e & 7) == 0) { double t = r.x; asm volatile("" : "+d"(t)); l2_discard128(a); }
+        return r;
+    };
+    auto st_c = [&](int e, cplx val) { stc_h(&dst[e], val, pol_c); };
     typedef FftPass<PL, 0> P0;
     if constexpr (PL::NPASS == 1) {
         if (active) {
@@ -237,23 +288,26 @@ __global__ void __launch_bounds__(NL* tpl8<PL>()) k_fft_y(DevParams P, const cpl
 // D[i][kz][j] contiguously.  Inverse = forward with re/im swapped on load and store.
 // ------------------------------------------------------------------------------------------
 template <class PL, int NL>
-__global__ void __launch_bounds__(NL* tpl8<PL>()) k_ifft_y(DevParams P, const cplx* __restrict__ T, cplx* __restrict__ D)
+__global__ void __launch_bounds__(NL* tpl8<PL>()) k_ifft_y(DevParams P, const cplx* __restrict__ T, cplx* __restrict__ D, int i_base, int np,
+                                                         int dmod)
 {
     constexpr int TPL = PL::TPL, LS = PL::LS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* sm = reinterpret_cast<cplx*>(smem_raw);
-    const int ngrp = (P.nx + NL - 1) / NL;
+    // this launch covers planes i_base .. i_base+np-1; D may be a rotating buffer of dmod planes
+    const int ngrp = (np + NL - 1) / NL;
     const int kz = blockIdx.x / ngrp, ig = blockIdx.x % ngrp;
     const int ln = (threadIdx.x >> 3) % NL;
     const int tl = (threadIdx.x & 7) | ((threadIdx.x / (8 * NL)) << 3);
-    const int i = ig * NL + ln;
-    const bool active = (i < P.nx) && (tl < TPL);
+    const int i = i_base + ig * NL + ln;
+    const bool active = (i < i_base + np) && (tl < TPL);
     const size_t tile_stride = (size_t)P.nx * 8;
     const cplx* src = T + (size_t)kz * (P.ny / 8) * tile_stride + (size_t)i * 8;
-    cplx* dst = D + ((size_t)i * P.nzh + kz) * (size_t)P.ny;
+    cplx* dst = D + ((size_t)(i % dmod) * P.nzh + kz) * (size_t)P.ny;
     cplx* line = sm + ln * LS;
-    auto ld_t = [&](int e) -> cplx { return cswap(__ldg(&src[(size_t)(e >> 3) * tile_stride + (e & 7)])); };
-    auto st_d = [&](int e, cplx val) { dst[e] = cswap(val); };
+    const unsigned long long pol_t = l2_policy((P.hints & 1) ? 1 : 0), pol_d = l2_policy((P.hints & 2) ? 2 : 0);
+    auto ld_t = [&](int e) -> cplx { return cswap(ldc_h(&src[(size_t)(e >> 3) * tile_stride + (e & 7)], pol_t)); };
+    auto st_d = [&](int e, cplx val) { stc_h(&dst[e], cswap(val), pol_d); };
     typedef FftPass<PL, 0> P0;
     if constexpr (PL::NPASS == 1) {
         if (active) {
@@ -280,20 +334,23 @@ __global__ void __launch_bounds__(NL* tpl8<PL>()) k_ifft_y(DevParams P, const cp
 // inverse complex FFT of length Nh gives z(m) = phi(2m) + i phi(2m+1).
 // ------------------------------------------------------------------------------------------
 template <class PL, int LPR>
-__global__ void __launch_bounds__(LPR* PL::TPL) k_c2r_z(DevParams P, const cplx* __restrict__ D, double* __restrict__ p)
+__global__ void __launch_bounds__(LPR* PL::TPL) k_c2r_z(DevParams P, const cplx* __restrict__ D, double* __restrict__ p, int i_base, int dmod)
 {
     constexpr int Nh = PL::N, TPL = PL::TPL, LS = PL::LS, NL = 8, NT = LPR * TPL;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* sm = reinterpret_cast<cplx*>(smem_raw);
     const int njt = P.ny / 8;
-    const int i = blockIdx.x / njt, jt = blockIdx.x % njt;
-    const cplx* src = D + (size_t)i * P.nzh * (size_t)P.ny + (size_t)jt * 8;
+    const int i = i_base + blockIdx.x / njt, jt = blockIdx.x % njt;
+    const cplx* src = D + (size_t)(i % dmod) * P.nzh * (size_t)P.ny + (size_t)jt * 8;
+    const unsigned long long pol_d = l2_policy((P.hints & 4) ? 1 : ((P.hints & 2) ? 2 : 0));
     for (int idx = threadIdx.x; idx < (Nh + 1) * NL; idx += NT) {
         const int k = idx >> 3, l = idx & 7;
-        cp_async16(&sm[l * LS + PL::pad(k)], &src[(size_t)k * P.ny + l]);
+        cp_async16h(&sm[l * LS + PL::pad(k)], &src[(size_t)k * P.ny + l], pol_d);
     }
     cp_async_wait_all();
     __syncthreads();
+    if (P.hints & 16) // the D lines of this tile are dead: drop them from L2 without a write-back
+        for (int k = threadIdx.x; k <= Nh; k += NT) l2_discard128(&src[(size_t)k * P.ny]);
     for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NT) {
         const int k = idx >> 3, l = idx & 7;
         const int km = Nh - k;
@@ -338,21 +395,23 @@ __global__ void __launch_bounds__(LPR* PL::TPL) k_c2r_z(DevParams P, const cplx*
 //   u[i] -= (phi[i]-phi[i-1])/dc_i (i >= 1; wall planes untouched), v -= d_y phi/dy, w -= d_z phi/dz.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_correct(DevParams P, const double* __restrict__ p, double* __restrict__ u,
-                                                 double* __restrict__ v, double* __restrict__ w)
+                                                 double* __restrict__ v, double* __restrict__ w, int i_base, int np)
 {
+    // this launch covers planes i_base .. i_base+np-1.
     // work order: j-chunks of JC lines outermost, then i, then the line inside the chunk, so that
     // plane i-1 of p (read again for the x-gradient) is still in L2 when plane i is processed
     const int nzh2 = P.nz / 2;
     constexpr int JC = 32;
-    const size_t npair = (size_t)P.nx * P.ny * nzh2;
+    const size_t npair = (size_t)np * P.ny * nzh2;
     const size_t plane = (size_t)P.ny * P.nz;
-    const size_t chunk_pairs = (size_t)P.nx * JC * nzh2;
+    const size_t chunk_pairs = (size_t)np * JC * nzh2;
+    const unsigned long long pol_in = l2_policy((P.hints & 1) ? 1 : 0), pol_out = l2_policy((P.hints & 8) ? 1 : 0);
     for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < npair; t += (size_t)gridDim.x * blockDim.x) {
         const int chunk = (int)(t / chunk_pairs);
         const size_t rem = t % chunk_pairs;
         const int jc_here = min(JC, P.ny - chunk * JC);
         const size_t slab = (size_t)jc_here * nzh2;
-        const int i = (int)(rem / slab);
+        const int i = i_base + (int)(rem / slab);
         const size_t r2 = rem % slab;
         const int j = chunk * JC + (int)(r2 / nzh2);
         const int kp = (int)(r2 % nzh2);
@@ -362,20 +421,20 @@ __global__ void __launch_bounds__(256) k_correct(DevParams P, const double* __re
         const size_t ojm = (j == 0) ? o + (size_t)(P.ny - 1) * P.nz : o - P.nz;
         const double2 pj = ldg2(p + ojm);
         const double pk = __ldg(p + (kp == 0 ? ij * P.nz + P.nz - 1 : o - 1));
-        double2 vv = *reinterpret_cast<double2*>(v + o), ww = *reinterpret_cast<double2*>(w + o);
+        double2 vv = ldc_h(reinterpret_cast<const cplx*>(v + o), pol_in), ww = ldc_h(reinterpret_cast<const cplx*>(w + o), pol_in);
         vv.x -= (ph.x - pj.x) * P.rdy;
         vv.y -= (ph.y - pj.y) * P.rdy;
         ww.x -= (ph.x - pk) * P.rdz;
         ww.y -= (ph.y - ph.x) * P.rdz;
-        *reinterpret_cast<double2*>(v + o) = vv;
-        *reinterpret_cast<double2*>(w + o) = ww;
+        stc_h(reinterpret_cast<cplx*>(v + o), vv, pol_out);
+        stc_h(reinterpret_cast<cplx*>(w + o), ww, pol_out);
         if (i >= 1) {
             const double2 pi = ldg2(p + o - plane);
             const double r = __ldg(&P.rdc[i]);
-            double2 uu = *reinterpret_cast<double2*>(u + o);
+            double2 uu = ldc_h(reinterpret_cast<const cplx*>(u + o), pol_in);
             uu.x -= (ph.x - pi.x) * r;
             uu.y -= (ph.y - pi.y) * r;
-            *reinterpret_cast<double2*>(u + o) = uu;
+            stc_h(reinterpret_cast<cplx*>(u + o), uu, pol_out);
         }
     }
 }

@@ -90,12 +90,16 @@ template <class PL> LaunchCfg cfg_k4()
 {
     return {(const void*)k_ifft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx), 3};
 }
+template <class PL> LaunchCfg cfg_k4s()
+{
+    return {(const void*)k_ifft_y<PL, 1>, tpl8<PL>(), (size_t)PL::LS * sizeof(cplx), 4};
+}
 template <class PL> LaunchCfg cfg_k5()
 {
     return {(const void*)k_c2r_z<PL, K5_LPR>, K5_LPR * PL::TPL, (size_t)8 * PL::LS * sizeof(cplx), 2};
 }
 
-bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4)
+bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4, LaunchCfg* k4s)
 {
     switch (n) {
 #define X(N, R0, R1, R2, R3, TPL)                   \
@@ -103,6 +107,7 @@ bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4)
         typedef FftPlan<R0, R1, R2, R3, TPL> PL;    \
         if (k2) *k2 = cfg_k2<PL>();                 \
         if (k4) *k4 = cfg_k4<PL>();                 \
+        if (k4s) *k4s = cfg_k4s<PL>();              \
         return true;                                \
     }
         AFID_FFT_SIZES(X)
@@ -139,13 +144,16 @@ struct afid_plan {
     size_t tables_bytes;
     cplx* ws[2];       // work arrays, nx*nzh*ny complex each
     size_t ws_bytes;
-    LaunchCfg k1, k2, k4, k5, k3;
+    LaunchCfg k1, k2, k4, k4s, k5, k3;
     int n_sm;
     // plane-batched forward sweep (K1 -> K2 through an L2-resident rotating B buffer)
     int s1_batch;      // planes per batch; 0 = one launch for all planes
     int s1_nstreams;
     cudaStream_t aux[8];
     cudaEvent_t ev_fork, ev_join[8];
+    // plane-batched inverse sweep (K4 -> K5 -> K6 through an L2-resident rotating D buffer)
+    int s2_batch;
+    cudaEvent_t ev_k5[8];
     // optional per-kernel timing (afid_plan_enable_timing): NK+1 events around the NK kernels
     bool timing;
     cudaEvent_t ev[7];
@@ -160,7 +168,7 @@ const char* afid_version(void) { return "afid-project-b200 0.1 (sm_100a, fp64)";
 const char* afid_last_error(void) { return g_err.c_str(); }
 int afid_last_error_code(void) { return g_err_code; }
 int afid_max_nx(void) { return MAX_NX; }
-int afid_fft_length_supported(int n) { return lookup_fft_y(n, nullptr, nullptr) ? 1 : 0; }
+int afid_fft_length_supported(int n) { return lookup_fft_y(n, nullptr, nullptr, nullptr) ? 1 : 0; }
 int afid_fft_half_length_supported(int n) { return lookup_fft_z(n, nullptr, nullptr) ? 1 : 0; }
 
 static int set_smem_attr(const LaunchCfg& c)
@@ -195,7 +203,7 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     afid_plan* pl = new (std::nothrow) afid_plan();
     if (!pl) { fail(AFID_ERR_NOMEM, "host allocation failed"); return nullptr; }
     std::memset(pl, 0, sizeof(*pl));
-    if (!lookup_fft_y(ny, &pl->k2, &pl->k4)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "ny is not a supported FFT length"); return nullptr; }
+    if (!lookup_fft_y(ny, &pl->k2, &pl->k4, &pl->k4s)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "ny is not a supported FFT length"); return nullptr; }
     if (!lookup_fft_z(nh, &pl->k1, &pl->k5)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "nz/2 is not a supported FFT length"); return nullptr; }
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
 
@@ -220,14 +228,16 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     pl->s1_nstreams = getenv("AFID_S1_STREAMS") ? atoi(getenv("AFID_S1_STREAMS")) : 3;
     if (pl->s1_nstreams < 1) pl->s1_nstreams = 1;
     if (pl->s1_nstreams > 8) pl->s1_nstreams = 8;
-    if (pl->s1_batch > 0) {
+    pl->s2_batch = getenv("AFID_S2_BATCH") ? atoi(getenv("AFID_S2_BATCH")) : 0;
+    if (pl->s1_batch > 0 || pl->s2_batch > 0) {
         cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming);
         for (int k = 0; k < pl->s1_nstreams; ++k) {
             cudaStreamCreateWithFlags(&pl->aux[k], cudaStreamNonBlocking);
             cudaEventCreateWithFlags(&pl->ev_join[k], cudaEventDisableTiming);
+            cudaEventCreateWithFlags(&pl->ev_k5[k], cudaEventDisableTiming);
         }
     }
-    for (const LaunchCfg* c : {&pl->k1, &pl->k2, &pl->k3, &pl->k4, &pl->k5}) {
+    for (const LaunchCfg* c : {&pl->k1, &pl->k2, &pl->k3, &pl->k4, &pl->k4s, &pl->k5}) {
         if (c->smem > prop.sharedMemPerBlockOptin) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "tile does not fit shared memory"); return nullptr; }
         if (set_smem_attr(*c) != AFID_OK) { delete pl; return nullptr; }
     }
@@ -302,6 +312,7 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     d.tw_zh = (const cplx*)(tb + items[8].off);
     d.tw_z = (const cplx*)(tb + items[9].off);
     d.inv_vol = (double)(1.0L / vol);
+    d.hints = getenv("AFID_HINTS") ? atoi(getenv("AFID_HINTS")) : 0;
     return pl;
 }
 
@@ -310,6 +321,14 @@ int afid_plan_destroy(afid_plan* pl)
     if (!pl) return AFID_OK;
     if (pl->timing)
         for (int k = 0; k < 7; ++k) cudaEventDestroy(pl->ev[k]);
+    if (pl->s1_batch > 0 || pl->s2_batch > 0) {
+        cudaEventDestroy(pl->ev_fork);
+        for (int k = 0; k < pl->s1_nstreams; ++k) {
+            cudaStreamDestroy(pl->aux[k]);
+            cudaEventDestroy(pl->ev_join[k]);
+            cudaEventDestroy(pl->ev_k5[k]);
+        }
+    }
     cudaFree(pl->ws[0]);
     cudaFree(pl->ws[1]);
     cudaFree(pl->tables);
@@ -388,6 +407,70 @@ static int run_solve(afid_plan* pl, const cplx* inC, cplx* outT, cudaStream_t st
     return launch(pl->k3, (unsigned)(pl->nzh * (pl->ny / 8)), st, args, "k_solve_x");
 }
 
+static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st)
+{
+    LaunchCfg c = {(const void*)k_correct, 256, 0, 0};
+    void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, &i_base, &np};
+    const size_t npair = (size_t)np * pl->ny * (pl->nz / 2);
+    size_t blocks = (npair + 255) / 256;
+    const size_t cap = (size_t)pl->n_sm * 64;
+    if (blocks > cap) blocks = cap;
+    return launch(c, (unsigned)blocks, st, args, "k_correct");
+}
+
+// K4 + K5 + K6: T -> D -> p, u, v, w
+static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double* v, double* w, double* p, cudaStream_t st,
+                       cudaEvent_t ev_a, cudaEvent_t ev_b)
+{
+    int rc;
+    if (pl->s2_batch <= 0) {
+        int i_base = 0, np = pl->nx, dmod = pl->nx;
+        {
+            void* args[] = {&pl->dp, (void*)&T, (void*)&D, &i_base, &np, &dmod};
+            if ((rc = launch(pl->k4, (unsigned)(pl->nzh * ((pl->nx + KY_NL - 1) / KY_NL)), st, args, "k_ifft_y"))) return rc;
+        }
+        if (ev_a) cudaEventRecord(ev_a, st);
+        {
+            void* args[] = {&pl->dp, (void*)&D, (void*)&p, &i_base, &dmod};
+            if ((rc = launch(pl->k5, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_z"))) return rc;
+        }
+        if (ev_b) cudaEventRecord(ev_b, st);
+        return launch_correct(pl, u, v, w, p, 0, pl->nx, st);
+    }
+    // plane-batched: batch k runs K4, K5, K6 on aux stream k % ns; D slot = stream index;
+    // K6 of batch k also needs plane i_base-1 of p, i.e. K5 of batch k-1 (event)
+    const int nb = pl->s2_batch, ns = pl->s1_nstreams;
+    int dmod = nb * ns;
+    cudaEventRecord(pl->ev_fork, st);
+    for (int k = 0; k < ns; ++k) cudaStreamWaitEvent(pl->aux[k], pl->ev_fork, 0);
+    int kb = 0;
+    for (int i_base = 0; i_base < pl->nx; i_base += nb, ++kb) {
+        int np = (pl->nx - i_base < nb) ? pl->nx - i_base : nb;
+        cudaStream_t s = pl->aux[kb % ns];
+        {
+            void* args[] = {&pl->dp, (void*)&T, (void*)&D, &i_base, &np, &dmod};
+            const bool pair = (np % KY_NL) == 0;
+            const LaunchCfg& c = pair ? pl->k4 : pl->k4s;
+            const int ngrp = pair ? np / KY_NL : np;
+            if ((rc = launch(c, (unsigned)(pl->nzh * ngrp), s, args, "k_ifft_y"))) return rc;
+        }
+        {
+            void* args[] = {&pl->dp, (void*)&D, (void*)&p, &i_base, &dmod};
+            if ((rc = launch(pl->k5, (unsigned)(np * (pl->ny / 8)), s, args, "k_c2r_z"))) return rc;
+        }
+        cudaEventRecord(pl->ev_k5[kb % ns], s);
+        if (kb > 0 && ns > 1) cudaStreamWaitEvent(s, pl->ev_k5[(kb - 1) % ns], 0);
+        if ((rc = launch_correct(pl, u, v, w, p, i_base, np, s))) return rc;
+    }
+    for (int k = 0; k < ns; ++k) {
+        cudaEventRecord(pl->ev_join[k], pl->aux[k]);
+        cudaStreamWaitEvent(st, pl->ev_join[k], 0);
+    }
+    if (ev_a) cudaEventRecord(ev_a, st);
+    if (ev_b) cudaEventRecord(ev_b, st);
+    return AFID_OK;
+}
+
 int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void* stream)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
@@ -402,25 +485,7 @@ int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void
     if (tm) cudaEventRecord(pl->ev[2], st);
     if ((rc = run_solve(pl, pl->ws[1], pl->ws[0], st))) return rc;             // T in ws0
     if (tm) cudaEventRecord(pl->ev[3], st);
-    {
-        void* args[] = {&pl->dp, (void*)&pl->ws[0], (void*)&pl->ws[1]};          // D in ws1
-        if ((rc = launch(pl->k4, (unsigned)(pl->nzh * ((pl->nx + KY_NL - 1) / KY_NL)), st, args, "k_ifft_y"))) return rc;
-    }
-    if (tm) cudaEventRecord(pl->ev[4], st);
-    {
-        void* args[] = {&pl->dp, (void*)&pl->ws[1], (void*)&p};
-        if ((rc = launch(pl->k5, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_z"))) return rc;
-    }
-    if (tm) cudaEventRecord(pl->ev[5], st);
-    {
-        LaunchCfg c = {(const void*)k_correct, 256, 0, 0};
-        void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w};
-        const size_t npair = (size_t)pl->nx * pl->ny * (pl->nz / 2);
-        size_t blocks = (npair + 255) / 256;
-        const size_t cap = (size_t)pl->n_sm * 64;
-        if (blocks > cap) blocks = cap;
-        if ((rc = launch(c, (unsigned)blocks, st, args, "k_correct"))) return rc;
-    }
+    if ((rc = run_inverse(pl, pl->ws[0], pl->ws[1], u, v, w, p, st, tm ? pl->ev[4] : nullptr, tm ? pl->ev[5] : nullptr))) return rc;
     if (tm) { cudaEventRecord(pl->ev[6], st); pl->ev_valid = true; }
     return AFID_OK;
 }
