@@ -391,50 +391,75 @@ __global__ void __launch_bounds__(LPR* PL::TPL) k_c2r_z(DevParams P, const cplx*
 }
 
 // ------------------------------------------------------------------------------------------
-// K6: correction.  One thread per pair of cells (k, k+1).
+// K6: correction.  CTA = (i, JL consecutive lines j); thread (x, y): line y, cell pairs
+// (2k, 2k+1) for k = x, x+TX, ... in batches of U pairs (all loads of a batch issued first).
 //   u[i] -= (phi[i]-phi[i-1])/dc_i (i >= 1; wall planes untouched), v -= d_y phi/dy, w -= d_z phi/dz.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_correct(DevParams P, const double* __restrict__ p, double* __restrict__ u,
-                                                 double* __restrict__ v, double* __restrict__ w, int i_base, int np)
+constexpr int K6_JL = 4, K6_TX = 64, K6_U = 4;
+
+__global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const double* __restrict__ p, double* __restrict__ u,
+                                                          double* __restrict__ v, double* __restrict__ w, int i_base, int np)
 {
+    constexpr int JL = K6_JL, TX = K6_TX, U = K6_U;
     // this launch covers planes i_base .. i_base+np-1.
-    // work order: j-chunks of JC lines outermost, then i, then the line inside the chunk, so that
+    // CTA order: j-chunks of 32 lines outermost, then i, then the group inside the chunk, so that
     // plane i-1 of p (read again for the x-gradient) is still in L2 when plane i is processed
-    const int nzh2 = P.nz / 2;
-    constexpr int JC = 32;
-    const size_t npair = (size_t)np * P.ny * nzh2;
+    const int ngrp = P.ny / JL;
+    constexpr int JC = 32 / JL;
+    const int per_chunk = np * JC;
+    int i, jg;
+    {
+        const int chunk = blockIdx.x / per_chunk, rem = blockIdx.x % per_chunk;
+        const int jc_here = min(JC, ngrp - chunk * JC);
+        i = i_base + rem / jc_here;
+        jg = chunk * JC + rem % jc_here;
+    }
+    const int j = jg * JL + threadIdx.y;
+    const int jm = (j == 0) ? P.ny - 1 : j - 1;
     const size_t plane = (size_t)P.ny * P.nz;
-    const size_t chunk_pairs = (size_t)np * JC * nzh2;
+    const size_t ol = ((size_t)i * P.ny + j) * P.nz;
+    const double* pl = p + ol;
+    const double* pjm = p + ((size_t)i * P.ny + jm) * P.nz;
+    const double* pim = pl - plane;          // only dereferenced for i >= 1
+    double *ul = u + ol, *vl = v + ol, *wl = w + ol;
+    const int nzh2 = P.nz / 2;
+    const bool has_u = (i >= 1);
+    const double rdc = has_u ? __ldg(&P.rdc[i]) : 0.0, rdy = P.rdy, rdz = P.rdz;
     const unsigned long long pol_in = l2_policy((P.hints & 1) ? 1 : 0), pol_out = l2_policy((P.hints & 8) ? 1 : 0);
-    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < npair; t += (size_t)gridDim.x * blockDim.x) {
-        const int chunk = (int)(t / chunk_pairs);
-        const size_t rem = t % chunk_pairs;
-        const int jc_here = min(JC, P.ny - chunk * JC);
-        const size_t slab = (size_t)jc_here * nzh2;
-        const int i = i_base + (int)(rem / slab);
-        const size_t r2 = rem % slab;
-        const int j = chunk * JC + (int)(r2 / nzh2);
-        const int kp = (int)(r2 % nzh2);
-        const size_t ij = (size_t)i * P.ny + j;
-        const size_t o = ij * P.nz + 2 * (size_t)kp;
-        const double2 ph = ldg2(p + o);
-        const size_t ojm = (j == 0) ? o + (size_t)(P.ny - 1) * P.nz : o - P.nz;
-        const double2 pj = ldg2(p + ojm);
-        const double pk = __ldg(p + (kp == 0 ? ij * P.nz + P.nz - 1 : o - 1));
-        double2 vv = ldc_h(reinterpret_cast<const cplx*>(v + o), pol_in), ww = ldc_h(reinterpret_cast<const cplx*>(w + o), pol_in);
-        vv.x -= (ph.x - pj.x) * P.rdy;
-        vv.y -= (ph.y - pj.y) * P.rdy;
-        ww.x -= (ph.x - pk) * P.rdz;
-        ww.y -= (ph.y - ph.x) * P.rdz;
-        stc_h(reinterpret_cast<cplx*>(v + o), vv, pol_out);
-        stc_h(reinterpret_cast<cplx*>(w + o), ww, pol_out);
-        if (i >= 1) {
-            const double2 pi = ldg2(p + o - plane);
-            const double r = __ldg(&P.rdc[i]);
-            double2 uu = ldc_h(reinterpret_cast<const cplx*>(u + o), pol_in);
-            uu.x -= (ph.x - pi.x) * r;
-            uu.y -= (ph.y - pi.y) * r;
-            stc_h(reinterpret_cast<cplx*>(u + o), uu, pol_out);
+    for (int k0 = threadIdx.x; k0 < nzh2; k0 += TX * U) {
+        double2 ph[U], pj[U], pi[U], uu[U], vv[U], ww[U];
+        double pk[U];
+#pragma unroll
+        for (int r = 0; r < U; ++r) {
+            const int kp = k0 + r * TX;
+            if (kp < nzh2) {
+                ph[r] = ldg2(pl + 2 * kp);
+                pj[r] = ldg2(pjm + 2 * kp);
+                pk[r] = __ldg(pl + (kp == 0 ? P.nz - 1 : 2 * kp - 1));
+                vv[r] = ldc_h(reinterpret_cast<const cplx*>(vl + 2 * kp), pol_in);
+                ww[r] = ldc_h(reinterpret_cast<const cplx*>(wl + 2 * kp), pol_in);
+                if (has_u) {
+                    pi[r] = ldg2(pim + 2 * kp);
+                    uu[r] = ldc_h(reinterpret_cast<const cplx*>(ul + 2 * kp), pol_in);
+                }
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < U; ++r) {
+            const int kp = k0 + r * TX;
+            if (kp < nzh2) {
+                vv[r].x -= (ph[r].x - pj[r].x) * rdy;
+                vv[r].y -= (ph[r].y - pj[r].y) * rdy;
+                ww[r].x -= (ph[r].x - pk[r]) * rdz;
+                ww[r].y -= (ph[r].y - ph[r].x) * rdz;
+                stc_h(reinterpret_cast<cplx*>(vl + 2 * kp), vv[r], pol_out);
+                stc_h(reinterpret_cast<cplx*>(wl + 2 * kp), ww[r], pol_out);
+                if (has_u) {
+                    uu[r].x -= (ph[r].x - pi[r].x) * rdc;
+                    uu[r].y -= (ph[r].y - pi[r].y) * rdc;
+                    stc_h(reinterpret_cast<cplx*>(ul + 2 * kp), uu[r], pol_out);
+                }
+            }
         }
     }
 }
@@ -472,13 +497,20 @@ __device__ __forceinline__ double fast_rcp(double x)
 }
 
 
-template <int M>
-__global__ void __launch_bounds__(M == 4 ? 128 : (M == 16 ? 512 : 384)) k_solve_x(DevParams P, const cplx* __restrict__ C, cplx* __restrict__ T)
+// EXACT: nx is a multiple of M (every chunk is full: no per-row bounds checks).
+// COEF_SMEM: the coefficients {a_i, c_i} are staged in shared memory (one conflict-free LDS.128 per
+// row instead of two global loads); not for the largest nx, where the tile fills shared memory.
+template <int M> constexpr int k3_threads() { return M == 4 ? 128 : (M == 16 ? 512 : 384); }
+__host__ __device__ constexpr int k3_coef_slots(int nx, int M) { return nx + nx / M + 1; }
+
+template <int M, bool EXACT, bool COEF_SMEM>
+__global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const cplx* __restrict__ C, cplx* __restrict__ T)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nx = P.nx, PCH = blockDim.x >> 3;
     cplx* tile = reinterpret_cast<cplx*>(smem_raw);            // [nx][8]
     double* red = reinterpret_cast<double*>(tile + (size_t)nx * 8); // 2 buffers x 5 arrays x [PCH][8]
+    double2* coef = reinterpret_cast<double2*>(red + 10 * PCH * 8);  // [nx + nx/M + 1] {a_i, c_i}, one pad slot per chunk
     const int nkt = P.ny / 8;
     const int kz = blockIdx.x / nkt, kyt = blockIdx.x % nkt;
     const int s = threadIdx.x & 7, q = threadIdx.x >> 3;
@@ -488,9 +520,15 @@ __global__ void __launch_bounds__(M == 4 ? 128 : (M == 16 ? 512 : 384)) k_solve_
         const cplx* src = C + (size_t)kz * P.ny + (size_t)kyt * 8 + s;
         const size_t rs = (size_t)P.nzh * P.ny;
         for (int i = q; i < nx; i += PCH) cp_async16(&tile[i * 8 + s], src + (size_t)i * rs);
+        if (COEF_SMEM)
+            for (int i = threadIdx.x; i < nx; i += blockDim.x) coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
         cp_async_wait_all();
         __syncthreads();
     }
+    auto ld_ac = [&](int i) -> double2 {
+        if (COEF_SMEM) return coef[i + i / M];
+        return make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
+    };
     const double lam = __ldg(&P.lamy[kyt * 8 + s]) + __ldg(&P.lamz[kz]);
     const bool cta_singular = (blockIdx.x == 0);
     const int i0 = q * M;
@@ -512,8 +550,9 @@ __global__ void __launch_bounds__(M == 4 ? 128 : (M == 16 ? 512 : 384)) k_solve_
 #pragma unroll
         for (int r = M - 2; r >= 0; --r) {
             const int i = i0 + r;
-            if (i < i1) {
-                const double a = __ldg(&P.ca[i]), c = __ldg(&P.cc[i]);
+            if (EXACT || i < i1) {
+                const double2 ac = ld_ac(i);
+                const double a = ac.x, c = ac.y;
                 const double nh = c * h, nt = fma(c, t, lam);
                 const double rr = fast_rcp(a + (nh + nt));
                 const cplx f = tile[i * 8 + s];
@@ -524,7 +563,7 @@ __global__ void __launch_bounds__(M == 4 ? 128 : (M == 16 ? 512 : 384)) k_solve_
             }
         }
         if (q > 0) { // contribution to the interface row above (reduced row q-1); staged in the "next" buffer
-            const double cb = __ldg(&P.cc[i0 - 1]);
+            const double cb = ld_ac(i0 - 1).y;
             nC[slot - 8] = cb * h;
             nL[slot - 8] = cb * t;
             nFr[slot - 8] = cb * yr;
@@ -539,8 +578,9 @@ __global__ void __launch_bounds__(M == 4 ? 128 : (M == 16 ? 512 : 384)) k_solve_
 #pragma unroll
         for (int r = 0; r < M - 1; ++r) {
             const int i = i0 + r;
-            if (i < i1) {
-                const double a = __ldg(&P.ca[i]), c = __ldg(&P.cc[i]);
+            if (EXACT || i < i1) {
+                const double2 ac = ld_ac(i);
+                const double a = ac.x, c = ac.y;
                 const double nh = a * h, nt = fma(a, t, lam);
                 const double rr = fast_rcp(c + (nh + nt));
                 const cplx f = tile[i * 8 + s];
@@ -553,7 +593,7 @@ __global__ void __launch_bounds__(M == 4 ? 128 : (M == 16 ? 512 : 384)) k_solve_
                 H[r] = h;
             }
         }
-        const double ab = __ldg(&P.ca[i1]);
+        const double ab = ld_ac(i1).x;
         const cplx f = tile[i1 * 8 + s];
         rA = ab * h;
         rL = fma(ab, t, lam);
@@ -617,7 +657,7 @@ __global__ void __launch_bounds__(M == 4 ? 128 : (M == 16 ? 512 : 384)) k_solve_
 #pragma unroll
         for (int r = M - 2; r >= 0; --r) {
             const int i = i0 + r;
-            if (i < i1) {
+            if (EXACT || i < i1) {
                 const cplx y = tile[i * 8 + s];
                 xr = fma(G[r], xr, fma(H[r], elr, y.x));
                 xi = fma(G[r], xi, fma(H[r], eli, y.y));

@@ -209,12 +209,13 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
 
     // ---- K3 configuration
     int M, pch;
-    if (nx < 64) { M = 4; pl->k3.fn = (const void*)k_solve_x<4>; }
-    else if (nx <= 1024) { M = 16; pl->k3.fn = (const void*)k_solve_x<16>; }
-    else { M = 32; pl->k3.fn = (const void*)k_solve_x<32>; }
+    if (nx < 64) { M = 4; pl->k3.fn = (nx % 4 == 0) ? (const void*)k_solve_x<4, true, true> : (const void*)k_solve_x<4, false, true>; }
+    else if (nx <= 1024) { M = 16; pl->k3.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true> : (const void*)k_solve_x<16, false, true>; }
+    else { M = 32; pl->k3.fn = (nx % 32 == 0) ? (const void*)k_solve_x<32, true, false> : (const void*)k_solve_x<32, false, false>; }
     pch = (nx + M - 1) / M;
     pl->k3.threads = 8 * pch;
-    pl->k3.smem = (size_t)nx * 8 * sizeof(cplx) + (size_t)10 * pch * 8 * sizeof(double);
+    pl->k3.smem = (size_t)nx * 8 * sizeof(cplx) + (size_t)10 * pch * 8 * sizeof(double)
+                  + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * sizeof(double2) : 0);
     pl->k3.ctas_per_sm = 4;
 
     int dev = 0;
@@ -409,13 +410,10 @@ static int run_solve(afid_plan* pl, const cplx* inC, cplx* outT, cudaStream_t st
 
 static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st)
 {
-    LaunchCfg c = {(const void*)k_correct, 256, 0, 0};
     void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, &i_base, &np};
-    const size_t npair = (size_t)np * pl->ny * (pl->nz / 2);
-    size_t blocks = (npair + 255) / 256;
-    const size_t cap = (size_t)pl->n_sm * 64;
-    if (blocks > cap) blocks = cap;
-    return launch(c, (unsigned)blocks, st, args, "k_correct");
+    cudaError_t e = cudaLaunchKernel((const void*)k_correct, dim3((unsigned)(np * (pl->ny / K6_JL))), dim3(K6_TX, K6_JL), args, 0, st);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_correct: ") + cudaGetErrorString(e));
+    return AFID_OK;
 }
 
 // K4 + K5 + K6: T -> D -> p, u, v, w
