@@ -13,11 +13,12 @@
 // segments (measured on B200: segmented reads of >=256 B run at copy speed, segmented
 // writes do not).  Work-array layouts (complex doubles; nzh = nz/2+1, NJT = ny/8):
 //   B  [i][jt][kz][8]     written by K1   (8 = j within the tile jt)
-//   C  [i][kz][ky]        written by K2
+//   C  [kz][i][ky]        written by K2   (kz-major: the rows i of a K3 tile are ny*16 bytes apart, not a plane apart)
 //   T  [kz][kyt][i][8]    written by K3   (8 = ky within the tile kyt)
 //   D  [i][kz][j]         written by K4
 #pragma once
 #include "fft_device.cuh"
+#include "tma.cuh"
 
 namespace afid {
 
@@ -233,7 +234,7 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
 
 // ------------------------------------------------------------------------------------------
 // K2: forward complex FFT along y.  CTA = (i, NL consecutive kz); reads B (segments of
-// NL*128 bytes), writes C[i][kz][ky] contiguously.
+// NL*128 bytes), writes C[kz][i][ky] contiguously.
 // ------------------------------------------------------------------------------------------
 template <class PL> constexpr int tpl8() { return (PL::TPL + 7) / 8 * 8; }
 
@@ -253,7 +254,7 @@ __global__ void __launch_bounds__(NL* tpl8<PL>()) k_fft_y(DevParams P, const cpl
     const bool active = (kz < P.nzh) && (tl < TPL);
     const cplx* src = B + (size_t)(i % bmod) * (P.ny / 8) * (size_t)P.nzh * 8 + (size_t)kz * 8;
     const size_t tile_stride = (size_t)P.nzh * 8;
-    cplx* dst = C + ((size_t)i * P.nzh + kz) * (size_t)P.ny;
+    cplx* dst = C + ((size_t)kz * P.nx + i) * (size_t)P.ny;
     cplx* line = sm + ln * LS;
     const unsigned long long pol_b = l2_policy((P.hints & 4) ? 1 : ((P.hints & 2) ? 2 : 0));
     const unsigned long long pol_c = l2_policy((P.hints & 8) ? 1 : 0);
@@ -333,60 +334,78 @@ __global__ void __launch_bounds__(NL* tpl8<PL>()) k_ifft_y(DevParams P, const cp
 //   Z'(k) = (X(k)+conj X(Nh-k)) + i conj(w^k)(X(k)-conj X(Nh-k)),
 // inverse complex FFT of length Nh gives z(m) = phi(2m) + i phi(2m+1).
 // ------------------------------------------------------------------------------------------
-template <class PL, int LPR>
-__global__ void __launch_bounds__(LPR* PL::TPL) k_c2r_z(DevParams P, const cplx* __restrict__ D, double* __restrict__ p, int i_base, int dmod)
+// TMA tile of K5: (Nh+1) rows kz of 128 bytes (8 j), fetched as k5_num_boxes boxes of k5_box_rows rows
+// (a multiple of 8, so that every box starts on a 1024-byte swizzle period); rows >= nz/2+1 are out of
+// bounds and arrive as zeros.  The shared-memory tile also has to hold the padded rows of the FFT passes.
+__host__ __device__ constexpr int k5_num_boxes(int nh) { return (nh + 1 + 255) / 256; }
+__host__ __device__ constexpr int k5_box_rows(int nh) { return ((nh + 1 + k5_num_boxes(nh) - 1) / k5_num_boxes(nh) + 7) / 8 * 8; }
+template <class PL> constexpr int k5_smem_rows()
 {
-    constexpr int Nh = PL::N, TPL = PL::TPL, LS = PL::LS, NL = 8, NT = LPR * TPL;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx* sm = reinterpret_cast<cplx*>(smem_raw);
+    constexpr int tma_rows = k5_num_boxes(PL::N) * k5_box_rows(PL::N);
+    constexpr int fft_rows = (PL::PADDED + 8) / 8 * 8;
+    return tma_rows > fft_rows ? tma_rows : fft_rows;
+}
+
+template <class PL, int LPR>
+__global__ void __launch_bounds__(LPR* PL::TPL, (LPR * PL::TPL <= 384) ? 2 : 1) k_c2r_z(DevParams P, const __grid_constant__ CUtensorMap mapD, double* __restrict__ p, int i_base,
+                                                        int dmod)
+{
+    constexpr int Nh = PL::N, TPL = PL::TPL, NL = 8, NT = LPR * TPL;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bar;
+    // 1024-byte aligned tile [row][8 chunks of 16 bytes]; line l, row r lives in chunk l ^ (r & 7)
+    // (the 128-byte TMA swizzle, kept for the in-place FFT passes: conflict-free for unit-stride rows)
+    cplx* sm = reinterpret_cast<cplx*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     const int njt = P.ny / 8;
     const int i = i_base + blockIdx.x / njt, jt = blockIdx.x % njt;
-    const cplx* src = D + (size_t)(i % dmod) * P.nzh * (size_t)P.ny + (size_t)jt * 8;
-    const unsigned long long pol_d = l2_policy((P.hints & 4) ? 1 : ((P.hints & 2) ? 2 : 0));
-    for (int idx = threadIdx.x; idx < (Nh + 1) * NL; idx += NT) {
-        const int k = idx >> 3, l = idx & 7;
-        cp_async16h(&sm[l * LS + PL::pad(k)], &src[(size_t)k * P.ny + l], pol_d);
+    if (threadIdx.x == 0) {
+        mbar_init(&bar, 1);
+        fence_mbar_init();
     }
-    cp_async_wait_all();
     __syncthreads();
-    if (P.hints & 16) // the D lines of this tile are dead: drop them from L2 without a write-back
-        for (int k = threadIdx.x; k <= Nh; k += NT) l2_discard128(&src[(size_t)k * P.ny]);
+    if (threadIdx.x == 0) {
+        constexpr int nb = k5_num_boxes(Nh), br = k5_box_rows(Nh);
+        const unsigned long long pol = l2_policy((P.hints & 4) ? 1 : ((P.hints & 2) ? 2 : 0));
+        mbar_expect_tx(&bar, (uint32_t)(nb * br * 8 * sizeof(cplx)));
+        for (int b = 0; b < nb; ++b) tma_load_3d_hint(sm + (size_t)b * br * 8, &mapD, jt * 16, b * br, i % dmod, &bar, pol);
+    }
+    auto at = [sm](int l, int r) -> cplx& { return sm[(r << 3) + (l ^ (r & 7))]; };
+    mbar_wait(&bar, 0);
     for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NT) {
         const int k = idx >> 3, l = idx & 7;
         const int km = Nh - k;
-        cplx* zl = sm + l * LS;
-        const cplx xk = zl[PL::pad(k)];
-        const cplx xm = zl[PL::pad(km)];
+        const cplx xk = at(l, k);
+        const cplx xm = at(l, km);
         const cplx wk = __ldg(&P.tw_z[k]);
         // E = X(k) + conj X(Nh-k), O = X(k) - conj X(Nh-k)
         const cplx E = mk(xk.x + xm.x, xk.y - xm.y), O = mk(xk.x - xm.x, xk.y + xm.y);
         const cplx wo = mk(fma(wk.y, O.y, wk.x * O.x), fma(-wk.y, O.x, wk.x * O.y)); // conj(w) * O
         const cplx t = mk(-wo.y, wo.x);                                              // i conj(w) O
         // stored re/im-swapped: the inverse transform runs as a forward one on swapped data
-        zl[PL::pad(k)] = mk(E.y + t.y, E.x + t.x);
+        at(l, k) = mk(E.y + t.y, E.x + t.x);
         // Z'(Nh-k) = conj( E - i conj(w) O )
-        if (k != 0 && k != km) zl[PL::pad(km)] = mk(-(E.y - t.y), E.x - t.x);
+        if (k != 0 && k != km) at(l, km) = mk(-(E.y - t.y), E.x - t.x);
     }
     __syncthreads();
     const int lr = threadIdx.x / TPL, tl = threadIdx.x % TPL;
 #pragma unroll 1
     for (int rnd = 0; rnd < NL / LPR; ++rnd) {
         const int ln = rnd * LPR + lr;
-        cplx* line = sm + ln * LS;
         double* dst = p + ((size_t)i * P.ny + (size_t)jt * 8 + ln) * (size_t)P.nz;
         auto st_p = [&](int e, cplx val) { reinterpret_cast<double2*>(dst)[e] = cswap(val); };
+        auto acc = [sm, ln](int pe) -> cplx& { return sm[(pe << 3) + (ln ^ (pe & 7))]; };
         typedef FftPass<PL, 0> P0;
         {
             typename P0::Regs rg;
-            P0::load(rg, tl, [&](int e) { return line[PL::pad(e)]; });
+            P0::load(rg, tl, [&](int e) { return at(ln, e); });   // unpadded rows, as TMA delivered them
             if constexpr (PL::NPASS == 1) {
                 P0::compute_store(rg, tl, P.tw_zh, st_p);
             } else {
                 __syncthreads();
-                P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { line[PL::pad(e)] = val; });
+                P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { acc(PL::pad(e)) = val; });
             }
         }
-        if constexpr (PL::NPASS > 1) fft_tail_passes<PL, 1, false>(line, tl, true, P.tw_zh, st_p);
+        if constexpr (PL::NPASS > 1) fft_tail_passes_acc<PL, 1, false>(acc, tl, true, P.tw_zh, st_p);
     }
 }
 
@@ -503,28 +522,44 @@ __device__ __forceinline__ double fast_rcp(double x)
 template <int M> constexpr int k3_threads() { return M == 4 ? 128 : (M == 16 ? 512 : 384); }
 __host__ __device__ constexpr int k3_coef_slots(int nx, int M) { return nx + nx / M + 1; }
 
+// rows per TMA box of the K3 tile gather (box = 8 ky x 1 kz x k3_box_rows(nx) planes), and the rows the
+// boxes cover together (>= nx; the excess is out of bounds in i and arrives as zeros)
+__host__ __device__ constexpr int k3_num_boxes(int nx) { return (nx + 255) / 256; }
+__host__ __device__ constexpr int k3_box_rows(int nx) { return (nx + k3_num_boxes(nx) - 1) / k3_num_boxes(nx); }
+__host__ __device__ constexpr int k3_tile_rows(int nx) { return k3_num_boxes(nx) * k3_box_rows(nx); }
+
 template <int M, bool EXACT, bool COEF_SMEM>
-__global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const cplx* __restrict__ C, cplx* __restrict__ T)
+__global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const __grid_constant__ CUtensorMap mapC, cplx* __restrict__ T)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bar;
     const int nx = P.nx, PCH = blockDim.x >> 3;
-    cplx* tile = reinterpret_cast<cplx*>(smem_raw);            // [nx][8]
-    double* red = reinterpret_cast<double*>(tile + (size_t)nx * 8); // 2 buffers x 5 arrays x [PCH][8]
+    // [k3_tile_rows(nx)][8], 128-byte aligned by hand (TMA destination; the launch adds 128 bytes of slack)
+    cplx* tile = reinterpret_cast<cplx*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
+    double* red = reinterpret_cast<double*>(tile + (size_t)k3_tile_rows(nx) * 8); // 2 buffers x 5 arrays x [PCH][8]
     double2* coef = reinterpret_cast<double2*>(red + 10 * PCH * 8);  // [nx + nx/M + 1] {a_i, c_i}, one pad slot per chunk
     const int nkt = P.ny / 8;
     const int kz = blockIdx.x / nkt, kyt = blockIdx.x % nkt;
     const int s = threadIdx.x & 7, q = threadIdx.x >> 3;
     const int slot = q * 8 + s, NS = PCH * 8;
 
-    {   // gather the 8 columns: 128-byte segments of C[i][kz][ky]
-        const cplx* src = C + (size_t)kz * P.ny + (size_t)kyt * 8 + s;
-        const size_t rs = (size_t)P.nzh * P.ny;
-        for (int i = q; i < nx; i += PCH) cp_async16(&tile[i * 8 + s], src + (size_t)i * rs);
-        if (COEF_SMEM)
-            for (int i = threadIdx.x; i < nx; i += blockDim.x) coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
-        cp_async_wait_all();
+    // gather the 8 columns C[kz][0..nx)[8 kyt .. 8 kyt + 8): TMA boxes of 128-byte rows, one mbarrier
+    if (threadIdx.x == 0) {
+        mbar_init(&bar, 1);
+        fence_mbar_init();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int nb = k3_num_boxes(nx), br = k3_box_rows(nx);
+        const unsigned long long pol = l2_policy((P.hints & 1) ? 1 : 0);
+        mbar_expect_tx(&bar, (uint32_t)(nb * br * 8 * sizeof(cplx)));
+        for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * 8, &mapC, kyt * 16, b * br, kz, &bar, pol);
+    }
+    if (COEF_SMEM) {
+        for (int i = threadIdx.x; i < nx; i += blockDim.x) coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
         __syncthreads();
     }
+    mbar_wait(&bar, 0);
     auto ld_ac = [&](int i) -> double2 {
         if (COEF_SMEM) return coef[i + i / M];
         return make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
@@ -544,36 +579,88 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
     double* nFr = nA + 3 * NS;
     double* nFi = nA + 4 * NS;
 
-    // upward elimination of the interior (read only): relation of the first interior row
-    {
-        double h = 1.0, t = 0.0, yr = 0.0, yi = 0.0;
+    double G[M - 1 > 0 ? M - 1 : 1], H[M - 1 > 0 ? M - 1 : 1];
+    double rA, rC, rL, rFr, rFi;
+    // Interior elimination of the chunk in both directions.  Upward (read only): relation of the first
+    // interior row to the interface above.  Downward (in place: tile <- y), keeping g, h in registers.
+    // The two recurrences are independent dependency chains; for full chunks they are interleaved row
+    // by row (twice the instruction-level parallelism); the downward sweep overwrites f with y, so the
+    // f of the first (M-1)/2 rows is kept in registers for the upward sweep, which reaches them last.
+    constexpr bool INTERLEAVE = EXACT && (M <= 16);
+    if constexpr (INTERLEAVE) {
+        constexpr int NF = (M - 1) / 2 > 0 ? (M - 1) / 2 : 1;
+        cplx F[NF];
+        double hu = 1.0, tu = 0.0, yur = 0.0, yui = 0.0;
+        double hd = 1.0, td = 0.0, ydr = 0.0, ydi = 0.0;
 #pragma unroll
-        for (int r = M - 2; r >= 0; --r) {
-            const int i = i0 + r;
-            if (EXACT || i < i1) {
-                const double2 ac = ld_ac(i);
+        for (int k = 0; k < M - 1; ++k) {
+            {   // upward, row ru = M-2-k (rows 0..k-1 already hold y: take f from the register copy)
+                const int ru = M - 2 - k;
+                const double2 ac = ld_ac(i0 + ru);
                 const double a = ac.x, c = ac.y;
-                const double nh = c * h, nt = fma(c, t, lam);
+                const cplx f = (ru >= k) ? tile[(i0 + ru) * 8 + s] : F[ru < NF ? ru : 0];
+                const double nh = c * hu, nt = fma(c, tu, lam);
                 const double rr = fast_rcp(a + (nh + nt));
-                const cplx f = tile[i * 8 + s];
-                h = nh * rr;
-                t = nt * rr;
-                yr = fma(c, yr, f.x) * rr;
-                yi = fma(c, yi, f.y) * rr;
+                hu = nh * rr;
+                tu = nt * rr;
+                yur = fma(c, yur, f.x) * rr;
+                yui = fma(c, yui, f.y) * rr;
+            }
+            {   // downward, row k
+                const double2 ac = ld_ac(i0 + k);
+                const double a = ac.x, c = ac.y;
+                const cplx f = tile[(i0 + k) * 8 + s];
+                if (k < NF && k < (M - 1) / 2) F[k] = f;
+                const double nh = a * hd, nt = fma(a, td, lam);
+                const double rr = fast_rcp(c + (nh + nt));
+                hd = nh * rr;
+                td = nt * rr;
+                ydr = fma(a, ydr, f.x) * rr;
+                ydi = fma(a, ydi, f.y) * rr;
+                tile[(i0 + k) * 8 + s] = mk(ydr, ydi);
+                G[k] = c * rr;
+                H[k] = hd;
             }
         }
         if (q > 0) { // contribution to the interface row above (reduced row q-1); staged in the "next" buffer
             const double cb = ld_ac(i0 - 1).y;
-            nC[slot - 8] = cb * h;
-            nL[slot - 8] = cb * t;
-            nFr[slot - 8] = cb * yr;
-            nFi[slot - 8] = cb * yi;
+            nC[slot - 8] = cb * hu;
+            nL[slot - 8] = cb * tu;
+            nFr[slot - 8] = cb * yur;
+            nFi[slot - 8] = cb * yui;
         }
-    }
-    // downward elimination of the interior (in place: tile <- y), keeping g, h in registers
-    double G[M - 1 > 0 ? M - 1 : 1], H[M - 1 > 0 ? M - 1 : 1];
-    double rA, rC, rL, rFr, rFi;
-    {
+        const double ab = ld_ac(i1).x;
+        const cplx f = tile[i1 * 8 + s];
+        rA = ab * hd;
+        rL = fma(ab, td, lam);
+        rFr = fma(ab, ydr, f.x);
+        rFi = fma(ab, ydi, f.y);
+    } else {
+        {
+            double h = 1.0, t = 0.0, yr = 0.0, yi = 0.0;
+#pragma unroll
+            for (int r = M - 2; r >= 0; --r) {
+                const int i = i0 + r;
+                if (EXACT || i < i1) {
+                    const double2 ac = ld_ac(i);
+                    const double a = ac.x, c = ac.y;
+                    const double nh = c * h, nt = fma(c, t, lam);
+                    const double rr = fast_rcp(a + (nh + nt));
+                    const cplx f = tile[i * 8 + s];
+                    h = nh * rr;
+                    t = nt * rr;
+                    yr = fma(c, yr, f.x) * rr;
+                    yi = fma(c, yi, f.y) * rr;
+                }
+            }
+            if (q > 0) {
+                const double cb = ld_ac(i0 - 1).y;
+                nC[slot - 8] = cb * h;
+                nL[slot - 8] = cb * t;
+                nFr[slot - 8] = cb * yr;
+                nFi[slot - 8] = cb * yi;
+            }
+        }
         double h = 1.0, t = 0.0, yr = 0.0, yi = 0.0;
 #pragma unroll
         for (int r = 0; r < M - 1; ++r) {
@@ -653,6 +740,24 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
         __syncthreads();
         const double elr = (q > 0) ? bFr[slot - 8] : 0.0, eli = (q > 0) ? bFi[slot - 8] : 0.0;
         double xr = er, xi = ei;
+        // T[kz][kyt][i][8]: the tile is contiguous in global memory.  All CTAs but the one holding the
+        // mean mode store x straight from the back substitution (128-byte segments per row; the stores
+        // drain while the next CTA of this SM already loads its tile).
+        cplx* dst = T + ((size_t)kz * nkt + kyt) * (size_t)nx * 8;
+        if (!cta_singular) {
+            dst[i1 * 8 + s] = mk(xr, xi);
+#pragma unroll
+            for (int r = M - 2; r >= 0; --r) {
+                const int i = i0 + r;
+                if (EXACT || i < i1) {
+                    const cplx y = tile[i * 8 + s];
+                    xr = fma(G[r], xr, fma(H[r], elr, y.x));
+                    xi = fma(G[r], xi, fma(H[r], eli, y.y));
+                    dst[i * 8 + s] = mk(xr, xi);
+                }
+            }
+            return;
+        }
         tile[i1 * 8 + s] = mk(xr, xi);
 #pragma unroll
         for (int r = M - 2; r >= 0; --r) {
@@ -693,7 +798,7 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
         }
         __syncthreads();
     }
-    {   // contiguous store of the tile: T[kz][kyt][i][8]
+    {   // the mean-mode CTA: contiguous store of the tile
         cplx* dst = T + ((size_t)kz * nkt + kyt) * (size_t)nx * 8;
         for (int e = threadIdx.x; e < nx * 8; e += blockDim.x) dst[e] = tile[e];
     }

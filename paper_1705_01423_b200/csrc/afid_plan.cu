@@ -96,7 +96,7 @@ template <class PL> LaunchCfg cfg_k4s()
 }
 template <class PL> LaunchCfg cfg_k5()
 {
-    return {(const void*)k_c2r_z<PL, K5_LPR>, K5_LPR * PL::TPL, (size_t)8 * PL::LS * sizeof(cplx), 2};
+    return {(const void*)k_c2r_z<PL, K5_LPR>, K5_LPR * PL::TPL, (size_t)k5_smem_rows<PL>() * 8 * sizeof(cplx) + 1024, 2};
 }
 
 bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4, LaunchCfg* k4s)
@@ -135,6 +135,37 @@ bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5)
 
 constexpr int MAX_NX = 1536;
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point lookup (no link-time
+// dependency on libcuda, so the library still loads on a machine without a driver)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// 3-D fp64 tensor map over a complex array [d2][d1][d0/2 complex]; box = (b0 doubles, b1, b2)
+bool make_map3(CUtensorMap* m, void* base, uint64_t d0, uint64_t d1, uint64_t d2, uint32_t b0, uint32_t b1, uint32_t b2,
+               CUtensorMapSwizzle swz)
+{
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return false;
+    cuuint64_t dims[3] = {d0, d1, d2};
+    cuuint64_t strides[2] = {d0 * 8, d0 * d1 * 8};
+    cuuint32_t box[3] = {b0, b1, b2};
+    cuuint32_t es[3] = {1, 1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
+              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 } // namespace
 
 struct afid_plan {
@@ -145,6 +176,8 @@ struct afid_plan {
     cplx* ws[2];       // work arrays, nx*nzh*ny complex each
     size_t ws_bytes;
     LaunchCfg k1, k2, k4, k4s, k5, k3;
+    alignas(64) CUtensorMap mapC;   // K3's gather of C = ws[1] viewed as [nzh][nx][2 ny] doubles
+    alignas(64) CUtensorMap mapD;   // K5's gather of D = ws[1], same view, 128-byte swizzle
     int n_sm;
     // plane-batched forward sweep (K1 -> K2 through an L2-resident rotating B buffer)
     int s1_batch;      // planes per batch; 0 = one launch for all planes
@@ -214,8 +247,8 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     else { M = 32; pl->k3.fn = (nx % 32 == 0) ? (const void*)k_solve_x<32, true, false> : (const void*)k_solve_x<32, false, false>; }
     pch = (nx + M - 1) / M;
     pl->k3.threads = 8 * pch;
-    pl->k3.smem = (size_t)nx * 8 * sizeof(cplx) + (size_t)10 * pch * 8 * sizeof(double)
-                  + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * sizeof(double2) : 0);
+    pl->k3.smem = (size_t)k3_tile_rows(nx) * 8 * sizeof(cplx) + (size_t)10 * pch * 8 * sizeof(double)
+                  + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * sizeof(double2) : 0) + 128;
     pl->k3.ctas_per_sm = 4;
 
     int dev = 0;
@@ -296,6 +329,16 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
             if (b == 1) cudaFree(pl->ws[0]);
             cudaFree(pl->tables); delete pl; fail(AFID_ERR_NOMEM, "cudaMalloc(work arrays) failed"); return nullptr;
         }
+    if (!make_map3(&pl->mapC, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)nx, (uint64_t)pl->nzh, 16, (uint32_t)k3_box_rows(nx), 1,
+                   CU_TENSOR_MAP_SWIZZLE_NONE)) {
+        cudaFree(pl->ws[0]); cudaFree(pl->ws[1]); cudaFree(pl->tables); delete pl;
+        fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed"); return nullptr;
+    }
+    if (!make_map3(&pl->mapD, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)pl->nzh, (uint64_t)nx, 16, (uint32_t)k5_box_rows(nh), 1,
+                   CU_TENSOR_MAP_SWIZZLE_128B)) {
+        cudaFree(pl->ws[0]); cudaFree(pl->ws[1]); cudaFree(pl->tables); delete pl;
+        fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed"); return nullptr;
+    }
     char* tb = (char*)pl->tables;
     DevParams& d = pl->dp;
     d.nx = nx; d.ny = ny; d.nz = nz; d.nzh = nh + 1;
@@ -402,9 +445,10 @@ static int run_forward(afid_plan* pl, const double* u, const double* v, const do
     return AFID_OK;
 }
 
-static int run_solve(afid_plan* pl, const cplx* inC, cplx* outT, cudaStream_t st)
+// K3: C (always ws[1]: the tensor map is bound to it) -> T
+static int run_solve(afid_plan* pl, cplx* outT, cudaStream_t st)
 {
-    void* args[] = {&pl->dp, (void*)&inC, (void*)&outT};
+    void* args[] = {&pl->dp, (void*)&pl->mapC, (void*)&outT};
     return launch(pl->k3, (unsigned)(pl->nzh * (pl->ny / 8)), st, args, "k_solve_x");
 }
 
@@ -429,7 +473,7 @@ static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double*
         }
         if (ev_a) cudaEventRecord(ev_a, st);
         {
-            void* args[] = {&pl->dp, (void*)&D, (void*)&p, &i_base, &dmod};
+            void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&p, &i_base, &dmod};
             if ((rc = launch(pl->k5, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_z"))) return rc;
         }
         if (ev_b) cudaEventRecord(ev_b, st);
@@ -453,7 +497,7 @@ static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double*
             if ((rc = launch(c, (unsigned)(pl->nzh * ngrp), s, args, "k_ifft_y"))) return rc;
         }
         {
-            void* args[] = {&pl->dp, (void*)&D, (void*)&p, &i_base, &dmod};
+            void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&p, &i_base, &dmod};
             if ((rc = launch(pl->k5, (unsigned)(np * (pl->ny / 8)), s, args, "k_c2r_z"))) return rc;
         }
         cudaEventRecord(pl->ev_k5[kb % ns], s);
@@ -481,7 +525,7 @@ int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void
     if (tm) cudaEventRecord(pl->ev[0], st);
     if ((rc = run_forward(pl, u, v, w, wsB, wsC, st, tm ? pl->ev[1] : nullptr))) return rc;   // B in ws0, C in ws1
     if (tm) cudaEventRecord(pl->ev[2], st);
-    if ((rc = run_solve(pl, pl->ws[1], pl->ws[0], st))) return rc;             // T in ws0
+    if ((rc = run_solve(pl, pl->ws[0], st))) return rc;             // T in ws0
     if (tm) cudaEventRecord(pl->ev[3], st);
     if ((rc = run_inverse(pl, pl->ws[0], pl->ws[1], u, v, w, p, st, tm ? pl->ev[4] : nullptr, tm ? pl->ev[5] : nullptr))) return rc;
     if (tm) { cudaEventRecord(pl->ev[6], st); pl->ev_valid = true; }
@@ -520,26 +564,41 @@ const char* afid_plan_kernel_name(const afid_plan* pl, int k)
     return (k >= 0 && k < 6) ? KERNEL_NAMES[k] : "";
 }
 
-int afid_stage_forward(afid_plan* pl, const double* u, const double* v, const double* w, double* spec, void* stream)
+// The taps speak [i][kz][ky]; the work array C is [kz][i][ky]: small re-layout kernels (not on the hot path).
+__global__ void k_tap_C_to_api(DevParams P, const cplx* __restrict__ C, cplx* __restrict__ A, int to_api)
 {
-    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
-    int rc;
-    if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(spec, "spec"))) return rc;
-    return run_forward(pl, u, v, w, pl->ws[0], (cplx*)spec, (cudaStream_t)stream, nullptr);
+    const size_t n = (size_t)P.nx * P.nzh * P.ny;
+    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+        const int ky = (int)(t % P.ny);
+        const size_t r = t / P.ny;
+        const int kz = (int)(r % P.nzh), i = (int)(r / P.nzh);       // t indexes the API layout
+        const size_t c = ((size_t)kz * P.nx + i) * P.ny + ky;
+        if (to_api) A[t] = C[c];
+        else const_cast<cplx*>(C)[c] = A[t];
+    }
 }
-
-// in place on a C-layout array: K3 writes the T layout into ws0, then a re-layout kernel is
-// not needed for the tap: K4's inverse transform is not part of this stage, so the tap
-// copies T back to C order with a small gather kernel.
-__global__ void k_tap_T_to_C(DevParams P, const cplx* __restrict__ T, cplx* __restrict__ C)
+__global__ void k_tap_T_to_api(DevParams P, const cplx* __restrict__ T, cplx* __restrict__ A)
 {
     const size_t n = (size_t)P.nx * P.nzh * P.ny;
     for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
         const int ky = (int)(t % P.ny);
         const size_t r = t / P.ny;
         const int kz = (int)(r % P.nzh), i = (int)(r / P.nzh);
-        C[t] = T[(((size_t)kz * (P.ny / 8) + ky / 8) * P.nx + i) * 8 + (ky & 7)];
+        A[t] = T[(((size_t)kz * (P.ny / 8) + ky / 8) * P.nx + i) * 8 + (ky & 7)];
     }
+}
+
+int afid_stage_forward(afid_plan* pl, const double* u, const double* v, const double* w, double* spec, void* stream)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    int rc;
+    if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(spec, "spec"))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = run_forward(pl, u, v, w, pl->ws[0], pl->ws[1], st, nullptr))) return rc;
+    k_tap_C_to_api<<<pl->n_sm * 8, 256, 0, st>>>(pl->dp, pl->ws[1], (cplx*)spec, 1);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_tap_C_to_api: ") + cudaGetErrorString(e));
+    return AFID_OK;
 }
 
 int afid_stage_solve(afid_plan* pl, double* spec, void* stream)
@@ -548,10 +607,11 @@ int afid_stage_solve(afid_plan* pl, double* spec, void* stream)
     int rc;
     if ((rc = check_ptr(spec, "spec"))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    if ((rc = run_solve(pl, (const cplx*)spec, pl->ws[0], st))) return rc;
-    k_tap_T_to_C<<<pl->n_sm * 8, 256, 0, st>>>(pl->dp, pl->ws[0], (cplx*)spec);
+    k_tap_C_to_api<<<pl->n_sm * 8, 256, 0, st>>>(pl->dp, pl->ws[1], (cplx*)spec, 0);
+    if ((rc = run_solve(pl, pl->ws[0], st))) return rc;
+    k_tap_T_to_api<<<pl->n_sm * 8, 256, 0, st>>>(pl->dp, pl->ws[0], (cplx*)spec);
     cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_tap_T_to_C: ") + cudaGetErrorString(e));
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_tap: ") + cudaGetErrorString(e));
     return AFID_OK;
 }
 

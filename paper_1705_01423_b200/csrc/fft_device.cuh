@@ -227,25 +227,32 @@ template <class PL, int P> struct FftPass {
 // output goes back to `line` instead (st_last unused) and a barrier follows it.
 // Every thread of the CTA must call this (it contains __syncthreads()); threads with
 // active == false take part in the barriers only.
-template <class PL, int P, bool LAST_TO_SMEM, class StoreLast>
-__device__ __forceinline__ void fft_tail_passes(cplx* line, int tl, bool active, const cplx* __restrict__ tw,
-                                                StoreLast st_last)
+// `acc(pe)` returns a reference to padded slot pe = PL::pad(e) of the line (the caller chooses where
+// the slots live: a plain padded line, or a swizzled column of a TMA tile).
+template <class PL, int P, bool LAST_TO_SMEM, class Acc, class StoreLast>
+__device__ __forceinline__ void fft_tail_passes_acc(Acc acc, int tl, bool active, const cplx* __restrict__ tw, StoreLast st_last)
 {
     if constexpr (P < PL::NPASS) {
         typedef FftPass<PL, P> PS;
         typename PS::Regs rg;
         __syncthreads(); // previous pass's writes visible
-        if (active) PS::load(rg, tl, [&](int e) { return line[PL::pad(e)]; });
+        if (active) PS::load(rg, tl, [&](int e) { return acc(PL::pad(e)); });
         if constexpr (P == PL::NPASS - 1 && !LAST_TO_SMEM) {
             if (active) PS::compute_store(rg, tl, tw, st_last);
         } else {
             __syncthreads(); // all reads done before the in-place writes
-            if (active) PS::compute_store(rg, tl, tw, [&](int e, cplx v) { line[PL::pad(e)] = v; });
+            if (active) PS::compute_store(rg, tl, tw, [&](int e, cplx v) { acc(PL::pad(e)) = v; });
         }
-        fft_tail_passes<PL, P + 1, LAST_TO_SMEM>(line, tl, active, tw, st_last);
+        fft_tail_passes_acc<PL, P + 1, LAST_TO_SMEM>(acc, tl, active, tw, st_last);
     } else {
         if constexpr (LAST_TO_SMEM) __syncthreads();
     }
+}
+template <class PL, int P, bool LAST_TO_SMEM, class StoreLast>
+__device__ __forceinline__ void fft_tail_passes(cplx* line, int tl, bool active, const cplx* __restrict__ tw,
+                                                StoreLast st_last)
+{
+    fft_tail_passes_acc<PL, P, LAST_TO_SMEM>([line](int pe) -> cplx& { return line[pe]; }, tl, active, tw, st_last);
 }
 
 } // namespace afid
