@@ -355,7 +355,7 @@ __global__ void __launch_bounds__(LPR* PL::TPL, (LPR * PL::TPL <= 384) ? 2 : 1) 
     __shared__ __align__(8) uint64_t bar;
     // 1024-byte aligned tile [row][8 chunks of 16 bytes]; line l, row r lives in chunk l ^ (r & 7)
     // (the 128-byte TMA swizzle, kept for the in-place FFT passes: conflict-free for unit-stride rows)
-    cplx* sm = reinterpret_cast<cplx*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    cplx* sm = reinterpret_cast<cplx*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u)); // (offset form keeps the shared state space)
     const int njt = P.ny / 8;
     const int i = i_base + blockIdx.x / njt, jt = blockIdx.x % njt;
     if (threadIdx.x == 0) {
@@ -371,6 +371,7 @@ __global__ void __launch_bounds__(LPR* PL::TPL, (LPR * PL::TPL <= 384) ? 2 : 1) 
     }
     auto at = [sm](int l, int r) -> cplx& { return sm[(r << 3) + (l ^ (r & 7))]; };
     mbar_wait(&bar, 0);
+    if (P.hints & 32) return; // experiment: tile gather only
     for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NT) {
         const int k = idx >> 3, l = idx & 7;
         const int km = Nh - k;
@@ -504,10 +505,20 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const dou
 // Mode (0,0) (lam = 0, singular; R7): last row pinned to 0, then the dx-weighted
 // mean is subtracted.
 // ------------------------------------------------------------------------------------------
+// 1/x for a positive, normal x, to fp64 round-off.  The 64-bit MUFU (rcp.approx.f64, MUFU.RCP64H) is
+// what the x-solve was bound by on B200 (XU pipe at 160 % of its sustained peak in ncu), so the seed is a
+// 32-bit MUFU.RCP of the mantissa, moved between the formats with integer operations only (no F2F
+// conversions: they use the same slow pipe), followed by two Newton steps (2^-22 -> 2^-44 -> 2^-88).
 __device__ __forceinline__ double fast_rcp(double x)
 {
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    const int hi = __double2hiint(x), lo = __double2loint(x);
+    const unsigned fb = 0x3F800000u | ((unsigned)(hi & 0xFFFFF) << 3) | ((unsigned)lo >> 29); // 1.m as a float in [1, 2)
+    float rf;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"(__uint_as_float(fb)));                 // in (0.5, 1]
+    const unsigned rb = __float_as_uint(rf);
+    const int ex = (hi >> 20) & 0x7FF;
+    const int rexp = (int)(rb >> 23) + (1023 - 127) - (ex - 1023);
+    double r = __hiloint2double((rexp << 20) | (int)((rb >> 3) & 0xFFFFF), (int)(rb << 29));
     double e = fma(-x, r, 1.0);
     r = fma(r, e, r);
     e = fma(-x, r, 1.0);
@@ -528,20 +539,22 @@ __host__ __device__ constexpr int k3_num_boxes(int nx) { return (nx + 255) / 256
 __host__ __device__ constexpr int k3_box_rows(int nx) { return (nx + k3_num_boxes(nx) - 1) / k3_num_boxes(nx); }
 __host__ __device__ constexpr int k3_tile_rows(int nx) { return k3_num_boxes(nx) * k3_box_rows(nx); }
 
-template <int M, bool EXACT, bool COEF_SMEM>
-__global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const __grid_constant__ CUtensorMap mapC, cplx* __restrict__ T)
+// KW = systems (consecutive ky) per CTA: 8 (128-byte rows), or 4 (64-byte rows; half the shared memory, so that
+// two CTAs share an SM and one gathers while the other computes -- used when the 8-wide tile allows only one).
+template <int M, bool EXACT, bool COEF_SMEM, int KW>
+__global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams P, const __grid_constant__ CUtensorMap mapC, cplx* __restrict__ T)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
-    const int nx = P.nx, PCH = blockDim.x >> 3;
-    // [k3_tile_rows(nx)][8], 128-byte aligned by hand (TMA destination; the launch adds 128 bytes of slack)
-    cplx* tile = reinterpret_cast<cplx*>((reinterpret_cast<uintptr_t>(smem_raw) + 127) & ~(uintptr_t)127);
-    double* red = reinterpret_cast<double*>(tile + (size_t)k3_tile_rows(nx) * 8); // 2 buffers x 5 arrays x [PCH][8]
-    double2* coef = reinterpret_cast<double2*>(red + 10 * PCH * 8);  // [nx + nx/M + 1] {a_i, c_i}, one pad slot per chunk
-    const int nkt = P.ny / 8;
-    const int kz = blockIdx.x / nkt, kyt = blockIdx.x % nkt;
-    const int s = threadIdx.x & 7, q = threadIdx.x >> 3;
-    const int slot = q * 8 + s, NS = PCH * 8;
+    const int nx = P.nx, PCH = blockDim.x / KW;
+    // [k3_tile_rows(nx)][KW], 128-byte aligned by hand (TMA destination; the launch adds 128 bytes of slack)
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u)); // (offset form keeps the shared state space)
+    double* red = reinterpret_cast<double*>(tile + (size_t)k3_tile_rows(nx) * KW); // 2 buffers x 5 arrays x [PCH][KW]
+    double2* coef = reinterpret_cast<double2*>(red + 10 * PCH * KW);  // [nx + nx/M + 1] {a_i, c_i}, one pad slot per chunk
+    const int nkt = P.ny / 8, ntile = P.ny / KW;
+    const int kz = blockIdx.x / ntile, ky0 = (blockIdx.x % ntile) * KW;   // first ky of this CTA
+    const int s = threadIdx.x % KW, q = threadIdx.x / KW;
+    const int slot = q * KW + s, NS = PCH * KW;
 
     // gather the 8 columns C[kz][0..nx)[8 kyt .. 8 kyt + 8): TMA boxes of 128-byte rows, one mbarrier
     if (threadIdx.x == 0) {
@@ -552,19 +565,20 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
     if (threadIdx.x == 0) {
         const int nb = k3_num_boxes(nx), br = k3_box_rows(nx);
         const unsigned long long pol = l2_policy((P.hints & 1) ? 1 : 0);
-        mbar_expect_tx(&bar, (uint32_t)(nb * br * 8 * sizeof(cplx)));
-        for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * 8, &mapC, kyt * 16, b * br, kz, &bar, pol);
+        mbar_expect_tx(&bar, (uint32_t)(nb * br * KW * sizeof(cplx)));
+        for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * KW, &mapC, ky0 * 2, b * br, kz, &bar, pol);
     }
     if (COEF_SMEM) {
         for (int i = threadIdx.x; i < nx; i += blockDim.x) coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
         __syncthreads();
     }
     mbar_wait(&bar, 0);
+    if (P.hints & 32) return; // experiment: tile gather only
     auto ld_ac = [&](int i) -> double2 {
         if (COEF_SMEM) return coef[i + i / M];
         return make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
     };
-    const double lam = __ldg(&P.lamy[kyt * 8 + s]) + __ldg(&P.lamz[kz]);
+    const double lam = __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]);
     const bool cta_singular = (blockIdx.x == 0);
     const int i0 = q * M;
     const int i1 = min(i0 + M, nx) - 1; // interface row of this chunk
@@ -598,7 +612,7 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
                 const int ru = M - 2 - k;
                 const double2 ac = ld_ac(i0 + ru);
                 const double a = ac.x, c = ac.y;
-                const cplx f = (ru >= k) ? tile[(i0 + ru) * 8 + s] : F[ru < NF ? ru : 0];
+                const cplx f = (ru >= k) ? tile[(i0 + ru) * KW + s] : F[ru < NF ? ru : 0];
                 const double nh = c * hu, nt = fma(c, tu, lam);
                 const double rr = fast_rcp(a + (nh + nt));
                 hu = nh * rr;
@@ -609,7 +623,7 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
             {   // downward, row k
                 const double2 ac = ld_ac(i0 + k);
                 const double a = ac.x, c = ac.y;
-                const cplx f = tile[(i0 + k) * 8 + s];
+                const cplx f = tile[(i0 + k) * KW + s];
                 if (k < NF && k < (M - 1) / 2) F[k] = f;
                 const double nh = a * hd, nt = fma(a, td, lam);
                 const double rr = fast_rcp(c + (nh + nt));
@@ -617,20 +631,20 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
                 td = nt * rr;
                 ydr = fma(a, ydr, f.x) * rr;
                 ydi = fma(a, ydi, f.y) * rr;
-                tile[(i0 + k) * 8 + s] = mk(ydr, ydi);
+                tile[(i0 + k) * KW + s] = mk(ydr, ydi);
                 G[k] = c * rr;
                 H[k] = hd;
             }
         }
         if (q > 0) { // contribution to the interface row above (reduced row q-1); staged in the "next" buffer
             const double cb = ld_ac(i0 - 1).y;
-            nC[slot - 8] = cb * hu;
-            nL[slot - 8] = cb * tu;
-            nFr[slot - 8] = cb * yur;
-            nFi[slot - 8] = cb * yui;
+            nC[slot - KW] = cb * hu;
+            nL[slot - KW] = cb * tu;
+            nFr[slot - KW] = cb * yur;
+            nFi[slot - KW] = cb * yui;
         }
         const double ab = ld_ac(i1).x;
-        const cplx f = tile[i1 * 8 + s];
+        const cplx f = tile[i1 * KW + s];
         rA = ab * hd;
         rL = fma(ab, td, lam);
         rFr = fma(ab, ydr, f.x);
@@ -646,7 +660,7 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
                     const double a = ac.x, c = ac.y;
                     const double nh = c * h, nt = fma(c, t, lam);
                     const double rr = fast_rcp(a + (nh + nt));
-                    const cplx f = tile[i * 8 + s];
+                    const cplx f = tile[i * KW + s];
                     h = nh * rr;
                     t = nt * rr;
                     yr = fma(c, yr, f.x) * rr;
@@ -655,10 +669,10 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
             }
             if (q > 0) {
                 const double cb = ld_ac(i0 - 1).y;
-                nC[slot - 8] = cb * h;
-                nL[slot - 8] = cb * t;
-                nFr[slot - 8] = cb * yr;
-                nFi[slot - 8] = cb * yi;
+                nC[slot - KW] = cb * h;
+                nL[slot - KW] = cb * t;
+                nFr[slot - KW] = cb * yr;
+                nFi[slot - KW] = cb * yi;
             }
         }
         double h = 1.0, t = 0.0, yr = 0.0, yi = 0.0;
@@ -670,18 +684,18 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
                 const double a = ac.x, c = ac.y;
                 const double nh = a * h, nt = fma(a, t, lam);
                 const double rr = fast_rcp(c + (nh + nt));
-                const cplx f = tile[i * 8 + s];
+                const cplx f = tile[i * KW + s];
                 h = nh * rr;
                 t = nt * rr;
                 yr = fma(a, yr, f.x) * rr;
                 yi = fma(a, yi, f.y) * rr;
-                tile[i * 8 + s] = mk(yr, yi);
+                tile[i * KW + s] = mk(yr, yi);
                 G[r] = c * rr;
                 H[r] = h;
             }
         }
         const double ab = ld_ac(i1).x;
-        const cplx f = tile[i1 * 8 + s];
+        const cplx f = tile[i1 * KW + s];
         rA = ab * h;
         rL = fma(ab, t, lam);
         rFr = fma(ab, yr, f.x);
@@ -705,7 +719,7 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
         __syncthreads();
         double A2 = 0.0, C2 = 0.0;
         if (q - d >= 0) {
-            const int m = slot - 8 * d;
+            const int m = slot - KW * d;
             const double Am = bA[m], Lm = bL[m];
             const double al = rA * fast_rcp(Am + bC[m] + Lm);
             A2 = al * Am;
@@ -714,7 +728,7 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
             rFi = fma(al, bFi[m], rFi);
         }
         if (q + d < PCH) {
-            const int m = slot + 8 * d;
+            const int m = slot + KW * d;
             const double Cp = bC[m], Lp = bL[m];
             const double ga = rC * fast_rcp(bA[m] + Cp + Lp);
             C2 = ga * Cp;
@@ -738,19 +752,19 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
         bFr[slot] = er;
         bFi[slot] = ei;
         __syncthreads();
-        const double elr = (q > 0) ? bFr[slot - 8] : 0.0, eli = (q > 0) ? bFi[slot - 8] : 0.0;
+        const double elr = (q > 0) ? bFr[slot - KW] : 0.0, eli = (q > 0) ? bFi[slot - KW] : 0.0;
         double xr = er, xi = ei;
         // T[kz][kyt][i][8]: the tile is contiguous in global memory.  All CTAs but the one holding the
         // mean mode store x straight from the back substitution (128-byte segments per row; the stores
         // drain while the next CTA of this SM already loads its tile).
-        cplx* dst = T + ((size_t)kz * nkt + kyt) * (size_t)nx * 8;
+        cplx* dst = T + ((size_t)kz * nkt + ky0 / 8) * (size_t)nx * 8 + (ky0 % 8);
         if (!cta_singular) {
             dst[i1 * 8 + s] = mk(xr, xi);
 #pragma unroll
             for (int r = M - 2; r >= 0; --r) {
                 const int i = i0 + r;
                 if (EXACT || i < i1) {
-                    const cplx y = tile[i * 8 + s];
+                    const cplx y = tile[i * KW + s];
                     xr = fma(G[r], xr, fma(H[r], elr, y.x));
                     xi = fma(G[r], xi, fma(H[r], eli, y.y));
                     dst[i * 8 + s] = mk(xr, xi);
@@ -758,15 +772,15 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
             }
             return;
         }
-        tile[i1 * 8 + s] = mk(xr, xi);
+        tile[i1 * KW + s] = mk(xr, xi);
 #pragma unroll
         for (int r = M - 2; r >= 0; --r) {
             const int i = i0 + r;
             if (EXACT || i < i1) {
-                const cplx y = tile[i * 8 + s];
+                const cplx y = tile[i * KW + s];
                 xr = fma(G[r], xr, fma(H[r], elr, y.x));
                 xi = fma(G[r], xi, fma(H[r], eli, y.y));
-                tile[i * 8 + s] = mk(xr, xi);
+                tile[i * KW + s] = mk(xr, xi);
             }
         }
     }
@@ -776,7 +790,7 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
             double sr = 0.0, si = 0.0;
             for (int i = i0; i <= i1; ++i) {
                 const double wgt = __ldg(&P.dxw[i]);
-                const cplx x = tile[i * 8];
+                const cplx x = tile[i * KW];
                 sr = fma(x.x, wgt, sr);
                 si = fma(x.y, wgt, si);
             }
@@ -790,17 +804,17 @@ __global__ void __launch_bounds__(k3_threads<M>()) k_solve_x(DevParams P, const 
             sr *= P.inv_vol;
             si *= P.inv_vol;
             for (int i = i0; i <= i1; ++i) {
-                cplx x = tile[i * 8];
+                cplx x = tile[i * KW];
                 x.x -= sr;
                 x.y -= si;
-                tile[i * 8] = x;
+                tile[i * KW] = x;
             }
         }
         __syncthreads();
     }
     {   // the mean-mode CTA: contiguous store of the tile
-        cplx* dst = T + ((size_t)kz * nkt + kyt) * (size_t)nx * 8;
-        for (int e = threadIdx.x; e < nx * 8; e += blockDim.x) dst[e] = tile[e];
+        cplx* dst = T + ((size_t)kz * nkt + ky0 / 8) * (size_t)nx * 8 + (ky0 % 8);
+        for (int e = threadIdx.x; e < nx * KW; e += blockDim.x) dst[(e / KW) * 8 + (e % KW)] = tile[e];
     }
 }
 

@@ -176,6 +176,7 @@ struct afid_plan {
     cplx* ws[2];       // work arrays, nx*nzh*ny complex each
     size_t ws_bytes;
     LaunchCfg k1, k2, k4, k4s, k5, k3;
+    int k3_kw;         // systems per K3 CTA (8 or 4)
     alignas(64) CUtensorMap mapC;   // K3's gather of C = ws[1] viewed as [nzh][nx][2 ny] doubles
     alignas(64) CUtensorMap mapD;   // K5's gather of D = ws[1], same view, 128-byte swizzle
     int n_sm;
@@ -242,12 +243,23 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
 
     // ---- K3 configuration
     int M, pch;
-    if (nx < 64) { M = 4; pl->k3.fn = (nx % 4 == 0) ? (const void*)k_solve_x<4, true, true> : (const void*)k_solve_x<4, false, true>; }
-    else if (nx <= 1024) { M = 16; pl->k3.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true> : (const void*)k_solve_x<16, false, true>; }
-    else { M = 32; pl->k3.fn = (nx % 32 == 0) ? (const void*)k_solve_x<32, true, false> : (const void*)k_solve_x<32, false, false>; }
+    int kw = 8;
+    if (nx < 64) { M = 4; pl->k3.fn = (nx % 4 == 0) ? (const void*)k_solve_x<4, true, true, 8> : (const void*)k_solve_x<4, false, true, 8>; }
+    else if (nx <= 1024) {
+        M = 16;
+        // 8-wide tiles if two of them fit an SM, else 4-wide ones (two CTAs per SM: one gathers while the other computes)
+        const size_t smem8 = (size_t)k3_tile_rows(nx) * 8 * sizeof(cplx) + (size_t)10 * ((nx + 15) / 16) * 8 * sizeof(double)
+                             + (size_t)k3_coef_slots(nx, 16) * sizeof(double2) + 128;
+        if (2 * (smem8 + 1024) > 228 * 1024) kw = 4;
+        if (getenv("AFID_K3_KW")) kw = atoi(getenv("AFID_K3_KW")) == 4 ? 4 : 8;
+        if (kw == 8) pl->k3.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 8> : (const void*)k_solve_x<16, false, true, 8>;
+        else pl->k3.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 4> : (const void*)k_solve_x<16, false, true, 4>;
+    }
+    else { M = 32; pl->k3.fn = (nx % 32 == 0) ? (const void*)k_solve_x<32, true, false, 8> : (const void*)k_solve_x<32, false, false, 8>; }
     pch = (nx + M - 1) / M;
-    pl->k3.threads = 8 * pch;
-    pl->k3.smem = (size_t)k3_tile_rows(nx) * 8 * sizeof(cplx) + (size_t)10 * pch * 8 * sizeof(double)
+    pl->k3_kw = kw;
+    pl->k3.threads = kw * pch;
+    pl->k3.smem = (size_t)k3_tile_rows(nx) * kw * sizeof(cplx) + (size_t)10 * pch * kw * sizeof(double)
                   + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * sizeof(double2) : 0) + 128;
     pl->k3.ctas_per_sm = 4;
 
@@ -329,7 +341,7 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
             if (b == 1) cudaFree(pl->ws[0]);
             cudaFree(pl->tables); delete pl; fail(AFID_ERR_NOMEM, "cudaMalloc(work arrays) failed"); return nullptr;
         }
-    if (!make_map3(&pl->mapC, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)nx, (uint64_t)pl->nzh, 16, (uint32_t)k3_box_rows(nx), 1,
+    if (!make_map3(&pl->mapC, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)nx, (uint64_t)pl->nzh, 2 * (uint32_t)pl->k3_kw, (uint32_t)k3_box_rows(nx), 1,
                    CU_TENSOR_MAP_SWIZZLE_NONE)) {
         cudaFree(pl->ws[0]); cudaFree(pl->ws[1]); cudaFree(pl->tables); delete pl;
         fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed"); return nullptr;
@@ -449,7 +461,7 @@ static int run_forward(afid_plan* pl, const double* u, const double* v, const do
 static int run_solve(afid_plan* pl, cplx* outT, cudaStream_t st)
 {
     void* args[] = {&pl->dp, (void*)&pl->mapC, (void*)&outT};
-    return launch(pl->k3, (unsigned)(pl->nzh * (pl->ny / 8)), st, args, "k_solve_x");
+    return launch(pl->k3, (unsigned)(pl->nzh * (pl->ny / pl->k3_kw)), st, args, "k_solve_x");
 }
 
 static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st)
