@@ -30,7 +30,7 @@ METRIC = "fp64 projection Mpoints/s at 1024x1536x1536; % of B200 HBM roofline"
 UNIT = "Mpoints/s"
 # algorithmic HBM bytes per grid point of each kernel: fp64, complex = 16 B per 2 points
 ALG_BYTES_PER_POINT = {"k_div_r2c": 32.0, "k_fft_y": 16.0, "k_solve_x": 16.0, "k_ifft_y": 16.0, "k_c2r_z": 16.0,
-                       "k_correct": 56.0}
+                       "k_correct": 56.0, "k_c2r_correct": 64.0}
 PATH_ALG_BYTES_PER_POINT = 96.0   # strict minimum of the whole path
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "about 8 TB/s"
 

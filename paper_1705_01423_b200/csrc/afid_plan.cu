@@ -90,16 +90,16 @@ template <class PL> LaunchCfg cfg_k4()
 {
     return {(const void*)k_ifft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx), 3};
 }
-template <class PL> LaunchCfg cfg_k4s()
+template <class PL> LaunchCfg cfg_k56()
 {
-    return {(const void*)k_ifft_y<PL, 1>, tpl8<PL>(), (size_t)PL::LS * sizeof(cplx), 4};
+    return {(const void*)k_c2r_correct<PL, K5_LPR>, K5_LPR * PL::TPL, (size_t)k5_smem_rows<PL>() * 8 * sizeof(cplx) + 1024, 2};
 }
 template <class PL> LaunchCfg cfg_k5()
 {
     return {(const void*)k_c2r_z<PL, K5_LPR>, K5_LPR * PL::TPL, (size_t)k5_smem_rows<PL>() * 8 * sizeof(cplx) + 1024, 2};
 }
 
-bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4, LaunchCfg* k4s)
+bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4)
 {
     switch (n) {
 #define X(N, R0, R1, R2, R3, TPL)                   \
@@ -107,7 +107,6 @@ bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4, LaunchCfg* k4s)
         typedef FftPlan<R0, R1, R2, R3, TPL> PL;    \
         if (k2) *k2 = cfg_k2<PL>();                 \
         if (k4) *k4 = cfg_k4<PL>();                 \
-        if (k4s) *k4s = cfg_k4s<PL>();              \
         return true;                                \
     }
         AFID_FFT_SIZES(X)
@@ -116,7 +115,7 @@ bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4, LaunchCfg* k4s)
         return false;
     }
 }
-bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5)
+bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5, LaunchCfg* k56)
 {
     switch (n) {
 #define X(N, R0, R1, R2, R3, TPL)                   \
@@ -124,6 +123,7 @@ bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5)
         typedef FftPlan<R0, R1, R2, R3, TPL> PL;    \
         if (k1) *k1 = cfg_k1<PL>();                 \
         if (k5) *k5 = cfg_k5<PL>();                 \
+        if (k56) *k56 = cfg_k56<PL>();              \
         return true;                                \
     }
         AFID_FFT_SIZES_Z(X)
@@ -175,19 +175,14 @@ struct afid_plan {
     size_t tables_bytes;
     cplx* ws[2];       // work arrays, nx*nzh*ny complex each
     size_t ws_bytes;
-    LaunchCfg k1, k2, k4, k4s, k5, k3;
+    LaunchCfg k1, k2, k4, k5, k56, k3;
+    bool fuse56;       // K5 and K6 as one kernel (k_c2r_correct) with inter-CTA flags
+    unsigned* sync56;  // ticket + one flag per tile (device)
+    unsigned epoch;    // call counter: the value the flags of the current call take
     int k3_kw;         // systems per K3 CTA (8 or 4)
     alignas(64) CUtensorMap mapC;   // K3's gather of C = ws[1] viewed as [nzh][nx][2 ny] doubles
     alignas(64) CUtensorMap mapD;   // K5's gather of D = ws[1], same view, 128-byte swizzle
     int n_sm;
-    // plane-batched forward sweep (K1 -> K2 through an L2-resident rotating B buffer)
-    int s1_batch;      // planes per batch; 0 = one launch for all planes
-    int s1_nstreams;
-    cudaStream_t aux[8];
-    cudaEvent_t ev_fork, ev_join[8];
-    // plane-batched inverse sweep (K4 -> K5 -> K6 through an L2-resident rotating D buffer)
-    int s2_batch;
-    cudaEvent_t ev_k5[8];
     // optional per-kernel timing (afid_plan_enable_timing): NK+1 events around the NK kernels
     bool timing;
     cudaEvent_t ev[7];
@@ -195,6 +190,8 @@ struct afid_plan {
 };
 
 static const char* const KERNEL_NAMES[6] = {"k_div_r2c", "k_fft_y", "k_solve_x", "k_ifft_y", "k_c2r_z", "k_correct"};
+static const char* const KERNEL_NAMES_FUSED[5] = {"k_div_r2c", "k_fft_y", "k_solve_x", "k_ifft_y", "k_c2r_correct"};
+static bool fused_path(const afid_plan* pl) { return pl->fuse56; }
 
 extern "C" {
 
@@ -202,8 +199,8 @@ const char* afid_version(void) { return "afid-project-b200 0.1 (sm_100a, fp64)";
 const char* afid_last_error(void) { return g_err.c_str(); }
 int afid_last_error_code(void) { return g_err_code; }
 int afid_max_nx(void) { return MAX_NX; }
-int afid_fft_length_supported(int n) { return lookup_fft_y(n, nullptr, nullptr, nullptr) ? 1 : 0; }
-int afid_fft_half_length_supported(int n) { return lookup_fft_z(n, nullptr, nullptr) ? 1 : 0; }
+int afid_fft_length_supported(int n) { return lookup_fft_y(n, nullptr, nullptr) ? 1 : 0; }
+int afid_fft_half_length_supported(int n) { return lookup_fft_z(n, nullptr, nullptr, nullptr) ? 1 : 0; }
 
 static int set_smem_attr(const LaunchCfg& c)
 {
@@ -237,8 +234,8 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     afid_plan* pl = new (std::nothrow) afid_plan();
     if (!pl) { fail(AFID_ERR_NOMEM, "host allocation failed"); return nullptr; }
     std::memset(pl, 0, sizeof(*pl));
-    if (!lookup_fft_y(ny, &pl->k2, &pl->k4, &pl->k4s)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "ny is not a supported FFT length"); return nullptr; }
-    if (!lookup_fft_z(nh, &pl->k1, &pl->k5)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "nz/2 is not a supported FFT length"); return nullptr; }
+    if (!lookup_fft_y(ny, &pl->k2, &pl->k4)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "ny is not a supported FFT length"); return nullptr; }
+    if (!lookup_fft_z(nh, &pl->k1, &pl->k5, &pl->k56)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "nz/2 is not a supported FFT length"); return nullptr; }
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
 
     // ---- K3 configuration
@@ -270,20 +267,7 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     }
     if (prop.major != 10) { delete pl; fail(AFID_ERR_CUDA, "this library is built for sm_100a (B200) only"); return nullptr; }
     pl->n_sm = prop.multiProcessorCount;
-    pl->s1_batch = getenv("AFID_S1_BATCH") ? atoi(getenv("AFID_S1_BATCH")) : 0;
-    pl->s1_nstreams = getenv("AFID_S1_STREAMS") ? atoi(getenv("AFID_S1_STREAMS")) : 3;
-    if (pl->s1_nstreams < 1) pl->s1_nstreams = 1;
-    if (pl->s1_nstreams > 8) pl->s1_nstreams = 8;
-    pl->s2_batch = getenv("AFID_S2_BATCH") ? atoi(getenv("AFID_S2_BATCH")) : 0;
-    if (pl->s1_batch > 0 || pl->s2_batch > 0) {
-        cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming);
-        for (int k = 0; k < pl->s1_nstreams; ++k) {
-            cudaStreamCreateWithFlags(&pl->aux[k], cudaStreamNonBlocking);
-            cudaEventCreateWithFlags(&pl->ev_join[k], cudaEventDisableTiming);
-            cudaEventCreateWithFlags(&pl->ev_k5[k], cudaEventDisableTiming);
-        }
-    }
-    for (const LaunchCfg* c : {&pl->k1, &pl->k2, &pl->k3, &pl->k4, &pl->k4s, &pl->k5}) {
+    for (const LaunchCfg* c : {&pl->k1, &pl->k2, &pl->k3, &pl->k4, &pl->k5, &pl->k56}) {
         if (c->smem > prop.sharedMemPerBlockOptin) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "tile does not fit shared memory"); return nullptr; }
         if (set_smem_attr(*c) != AFID_OK) { delete pl; return nullptr; }
     }
@@ -334,6 +318,13 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
         if (cudaMemcpy((char*)pl->tables + it.off, it.src, it.bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
             cudaFree(pl->tables); delete pl; fail(AFID_ERR_CUDA, "cudaMemcpy(tables) failed"); return nullptr;
         }
+    pl->fuse56 = getenv("AFID_FUSE56") && atoi(getenv("AFID_FUSE56")) == 1; // off by default: slower than K5 + K6
+    {
+        const size_t nflag = 1 + (size_t)nx * (ny / 8);
+        if (cudaMalloc((void**)&pl->sync56, nflag * sizeof(unsigned)) != cudaSuccess || cudaMemset(pl->sync56, 0, nflag * sizeof(unsigned)) != cudaSuccess) {
+            cudaGetLastError(); cudaFree(pl->tables); delete pl; fail(AFID_ERR_NOMEM, "cudaMalloc(flags) failed"); return nullptr;
+        }
+    }
     pl->ws_bytes = (size_t)nx * pl->nzh * ny * sizeof(cplx);
     for (int b = 0; b < 2; ++b)
         if (cudaMalloc((void**)&pl->ws[b], pl->ws_bytes) != cudaSuccess) {
@@ -377,23 +368,16 @@ int afid_plan_destroy(afid_plan* pl)
     if (!pl) return AFID_OK;
     if (pl->timing)
         for (int k = 0; k < 7; ++k) cudaEventDestroy(pl->ev[k]);
-    if (pl->s1_batch > 0 || pl->s2_batch > 0) {
-        cudaEventDestroy(pl->ev_fork);
-        for (int k = 0; k < pl->s1_nstreams; ++k) {
-            cudaStreamDestroy(pl->aux[k]);
-            cudaEventDestroy(pl->ev_join[k]);
-            cudaEventDestroy(pl->ev_k5[k]);
-        }
-    }
     cudaFree(pl->ws[0]);
     cudaFree(pl->ws[1]);
     cudaFree(pl->tables);
+    cudaFree(pl->sync56);
     delete pl;
     return AFID_OK;
 }
 
 size_t afid_plan_workspace_bytes(const afid_plan* pl) { return pl ? 2 * pl->ws_bytes + pl->tables_bytes : 0; }
-int afid_plan_num_launches(const afid_plan* pl) { return pl ? 6 : 0; }
+int afid_plan_num_launches(const afid_plan* pl) { return pl ? (fused_path(pl) ? 5 : 6) : 0; }
 
 static int launch(const LaunchCfg& c, unsigned grid, cudaStream_t st, void** args, const char* name)
 {
@@ -415,46 +399,14 @@ static int run_forward(afid_plan* pl, const double* u, const double* v, const do
 {
     int rc;
     const int ngrp2 = (pl->nzh + KY_NL - 1) / KY_NL;
-    if (pl->s1_batch <= 0) {
-        int i_base = 0, np = pl->nx, bmod = pl->nx;
-        {
-            void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &i_base, &np, &bmod};
-            rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c");
-            if (rc) return rc;
-        }
-        if (ev_mid) cudaEventRecord(ev_mid, st);
-        {
-            void* args[] = {&pl->dp, (void*)&wsB, (void*)&outC, &i_base, &bmod};
-            rc = launch(pl->k2, (unsigned)(pl->nx * ngrp2), st, args, "k_fft_y");
-        }
-        return rc;
-    }
-    // plane-batched: batch k runs K1 then K2 on aux stream k % ns, B slot = stream index
-    const int nb = pl->s1_batch, ns = pl->s1_nstreams;
-    int bmod = nb * ns;
-    cudaEventRecord(pl->ev_fork, st);
-    for (int k = 0; k < ns; ++k) cudaStreamWaitEvent(pl->aux[k], pl->ev_fork, 0);
-    int kb = 0;
-    for (int i_base = 0; i_base < pl->nx; i_base += nb, ++kb) {
-        int np = (pl->nx - i_base < nb) ? pl->nx - i_base : nb;
-        cudaStream_t s = pl->aux[kb % ns];
-        {
-            void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &i_base, &np, &bmod};
-            rc = launch(pl->k1, (unsigned)(np * (pl->ny / K1_NL)), s, args, "k_div_r2c");
-            if (rc) return rc;
-        }
-        {
-            void* args[] = {&pl->dp, (void*)&wsB, (void*)&outC, &i_base, &bmod};
-            rc = launch(pl->k2, (unsigned)(np * ngrp2), s, args, "k_fft_y");
-            if (rc) return rc;
-        }
-    }
-    for (int k = 0; k < ns; ++k) {
-        cudaEventRecord(pl->ev_join[k], pl->aux[k]);
-        cudaStreamWaitEvent(st, pl->ev_join[k], 0);
+    int i_base = 0, np = pl->nx, bmod = pl->nx;
+    {
+        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &i_base, &np, &bmod};
+        if ((rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c"))) return rc;
     }
     if (ev_mid) cudaEventRecord(ev_mid, st);
-    return AFID_OK;
+    void* args[] = {&pl->dp, (void*)&wsB, (void*)&outC, &i_base, &bmod};
+    return launch(pl->k2, (unsigned)(pl->nx * ngrp2), st, args, "k_fft_y");
 }
 
 // K3: C (always ws[1]: the tensor map is bound to it) -> T
@@ -472,57 +424,28 @@ static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double
     return AFID_OK;
 }
 
-// K4 + K5 + K6: T -> D -> p, u, v, w
+// K4 + K5 + K6 (or K4 + the fused K5/K6): T -> D -> p, u, v, w
 static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double* v, double* w, double* p, cudaStream_t st,
                        cudaEvent_t ev_a, cudaEvent_t ev_b)
 {
     int rc;
-    if (pl->s2_batch <= 0) {
-        int i_base = 0, np = pl->nx, dmod = pl->nx;
-        {
-            void* args[] = {&pl->dp, (void*)&T, (void*)&D, &i_base, &np, &dmod};
-            if ((rc = launch(pl->k4, (unsigned)(pl->nzh * ((pl->nx + KY_NL - 1) / KY_NL)), st, args, "k_ifft_y"))) return rc;
-        }
-        if (ev_a) cudaEventRecord(ev_a, st);
-        {
-            void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&p, &i_base, &dmod};
-            if ((rc = launch(pl->k5, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_z"))) return rc;
-        }
-        if (ev_b) cudaEventRecord(ev_b, st);
-        return launch_correct(pl, u, v, w, p, 0, pl->nx, st);
-    }
-    // plane-batched: batch k runs K4, K5, K6 on aux stream k % ns; D slot = stream index;
-    // K6 of batch k also needs plane i_base-1 of p, i.e. K5 of batch k-1 (event)
-    const int nb = pl->s2_batch, ns = pl->s1_nstreams;
-    int dmod = nb * ns;
-    cudaEventRecord(pl->ev_fork, st);
-    for (int k = 0; k < ns; ++k) cudaStreamWaitEvent(pl->aux[k], pl->ev_fork, 0);
-    int kb = 0;
-    for (int i_base = 0; i_base < pl->nx; i_base += nb, ++kb) {
-        int np = (pl->nx - i_base < nb) ? pl->nx - i_base : nb;
-        cudaStream_t s = pl->aux[kb % ns];
-        {
-            void* args[] = {&pl->dp, (void*)&T, (void*)&D, &i_base, &np, &dmod};
-            const bool pair = (np % KY_NL) == 0;
-            const LaunchCfg& c = pair ? pl->k4 : pl->k4s;
-            const int ngrp = pair ? np / KY_NL : np;
-            if ((rc = launch(c, (unsigned)(pl->nzh * ngrp), s, args, "k_ifft_y"))) return rc;
-        }
-        {
-            void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&p, &i_base, &dmod};
-            if ((rc = launch(pl->k5, (unsigned)(np * (pl->ny / 8)), s, args, "k_c2r_z"))) return rc;
-        }
-        cudaEventRecord(pl->ev_k5[kb % ns], s);
-        if (kb > 0 && ns > 1) cudaStreamWaitEvent(s, pl->ev_k5[(kb - 1) % ns], 0);
-        if ((rc = launch_correct(pl, u, v, w, p, i_base, np, s))) return rc;
-    }
-    for (int k = 0; k < ns; ++k) {
-        cudaEventRecord(pl->ev_join[k], pl->aux[k]);
-        cudaStreamWaitEvent(st, pl->ev_join[k], 0);
+    int i_base = 0, np = pl->nx, dmod = pl->nx;
+    {
+        void* args[] = {&pl->dp, (void*)&T, (void*)&D, &i_base, &np, &dmod};
+        if ((rc = launch(pl->k4, (unsigned)(pl->nzh * ((pl->nx + KY_NL - 1) / KY_NL)), st, args, "k_ifft_y"))) return rc;
     }
     if (ev_a) cudaEventRecord(ev_a, st);
+    if (pl->fuse56) {
+        unsigned epoch = ++pl->epoch;
+        void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&p, (void*)&u, (void*)&v, (void*)&w, (void*)&pl->sync56, &epoch};
+        return launch(pl->k56, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_correct");
+    }
+    {
+        void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&p, &i_base, &dmod};
+        if ((rc = launch(pl->k5, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_z"))) return rc;
+    }
     if (ev_b) cudaEventRecord(ev_b, st);
-    return AFID_OK;
+    return launch_correct(pl, u, v, w, p, 0, pl->nx, st);
 }
 
 int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void* stream)
@@ -565,14 +488,18 @@ int afid_plan_kernel_times(afid_plan* pl, float* ms, int n)
     if (!pl || !ms) return fail(AFID_ERR_NULL, "plan or ms is NULL");
     if (!pl->timing || !pl->ev_valid) return fail(AFID_ERR_CUDA, "timing not enabled or no projection recorded");
     if (cudaEventSynchronize(pl->ev[6]) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventSynchronize failed");
-    for (int k = 0; k < 6 && k < n; ++k)
-        if (cudaEventElapsedTime(&ms[k], pl->ev[k], pl->ev[k + 1]) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventElapsedTime failed");
+    const int nk = fused_path(pl) ? 5 : 6;
+    for (int k = 0; k < nk && k < n; ++k) {
+        // fused path: the last kernel runs from ev[4] to ev[6] (ev[5] is not recorded)
+        cudaEvent_t e1 = (nk == 5 && k == 4) ? pl->ev[6] : pl->ev[k + 1];
+        if (cudaEventElapsedTime(&ms[k], pl->ev[k], e1) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventElapsedTime failed");
+    }
     return AFID_OK;
 }
 
 const char* afid_plan_kernel_name(const afid_plan* pl, int k)
 {
-    (void)pl;
+    if (pl && fused_path(pl)) return (k >= 0 && k < 5) ? KERNEL_NAMES_FUSED[k] : "";
     return (k >= 0 && k < 6) ? KERNEL_NAMES[k] : "";
 }
 
