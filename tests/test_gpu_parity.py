@@ -189,6 +189,9 @@ def _full_size_checks(name, sample_planes):
     nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
     nzh = nz // 2 + 1
     need = (4 * nx * ny * nz * 8 + 2 * nx * nzh * ny * 16) * 1.35
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()          # give back what earlier tests' caches still hold
     free, _ = torch.cuda.mem_get_info()
     if free < need:
         pytest.skip(f"{name} needs {need / 2**30:.0f} GiB of device memory")
