@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
 template <class PL> constexpr int tpl8() { return (PL::TPL + 7) / 8 * 8; }
 
 template <class PL, int NL>
-__global__ void __launch_bounds__(NL* tpl8<PL>(), (NL * tpl8<PL>() <= 192) ? 3 : 1) k_fft_y(DevParams P, const cplx* __restrict__ B, cplx* __restrict__ C, int i_base, int bmod)
+__global__ void __launch_bounds__(NL* tpl8<PL>(), (NL * tpl8<PL>() <= 192) ? 3 : ((NL * tpl8<PL>() <= 256) ? 2 : 1)) k_fft_y(DevParams P, const cplx* __restrict__ B, cplx* __restrict__ C, int i_base, int bmod)
 {
     constexpr int TPL = PL::TPL, LS = PL::LS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -286,7 +286,7 @@ __global__ void __launch_bounds__(NL* tpl8<PL>(), (NL * tpl8<PL>() <= 192) ? 3 :
 // D[i][kz][j] contiguously.  Inverse = forward with re/im swapped on load and store.
 // ------------------------------------------------------------------------------------------
 template <class PL, int NL>
-__global__ void __launch_bounds__(NL* tpl8<PL>(), (NL * tpl8<PL>() <= 192) ? 3 : 1) k_ifft_y(DevParams P, const cplx* __restrict__ T, cplx* __restrict__ D, int i_base, int np,
+__global__ void __launch_bounds__(NL* tpl8<PL>(), (NL * tpl8<PL>() <= 192) ? 3 : ((NL * tpl8<PL>() <= 256) ? 2 : 1)) k_ifft_y(DevParams P, const cplx* __restrict__ T, cplx* __restrict__ D, int i_base, int np,
                                                          int dmod)
 {
     constexpr int TPL = PL::TPL, LS = PL::LS;

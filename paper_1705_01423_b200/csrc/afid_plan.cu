@@ -69,13 +69,16 @@ int fail(int code, const std::string& msg)
 
 constexpr int K1_NL = 4; // lines per CTA in K1 (two CTAs fill one 128-byte row of B)
 constexpr int K5_LPR = 4; // lines per round in K5 (8 lines per CTA, 2 rounds)
-constexpr int KY_NL = 2; // lines per CTA in K2 / K4 (256-byte gather segments)
+// lines per CTA in K2 / K4: 2 (256-byte gather segments), 1 for the longest lines (two 256-thread CTAs per SM
+// instead of one 512-thread CTA)
+template <class PL> constexpr int ky_nl() { return tpl8<PL>() >= 256 ? 1 : 2; }
 
 struct LaunchCfg {
     const void* fn;
     int threads;
     size_t smem;
     int ctas_per_sm; // CTAs per SM the shared-memory carveout is sized for (the rest stays L1)
+    int nl;          // lines per CTA (K2 / K4)
 };
 
 template <class PL> LaunchCfg cfg_k1()
@@ -84,11 +87,11 @@ template <class PL> LaunchCfg cfg_k1()
 }
 template <class PL> LaunchCfg cfg_k2()
 {
-    return {(const void*)k_fft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx), 3};
+    return {(const void*)k_fft_y<PL, ky_nl<PL>()>, ky_nl<PL>() * tpl8<PL>(), (size_t)ky_nl<PL>() * PL::LS * sizeof(cplx), 3, ky_nl<PL>()};
 }
 template <class PL> LaunchCfg cfg_k4()
 {
-    return {(const void*)k_ifft_y<PL, KY_NL>, KY_NL * tpl8<PL>(), (size_t)KY_NL * PL::LS * sizeof(cplx), 3};
+    return {(const void*)k_ifft_y<PL, ky_nl<PL>()>, ky_nl<PL>() * tpl8<PL>(), (size_t)ky_nl<PL>() * PL::LS * sizeof(cplx), 3, ky_nl<PL>()};
 }
 template <class PL> LaunchCfg cfg_k56()
 {
@@ -398,7 +401,7 @@ static int run_forward(afid_plan* pl, const double* u, const double* v, const do
                        cudaEvent_t ev_mid)
 {
     int rc;
-    const int ngrp2 = (pl->nzh + KY_NL - 1) / KY_NL;
+    const int ngrp2 = (pl->nzh + pl->k2.nl - 1) / pl->k2.nl;
     int i_base = 0, np = pl->nx, bmod = pl->nx;
     {
         void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &i_base, &np, &bmod};
@@ -432,7 +435,7 @@ static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double*
     int i_base = 0, np = pl->nx, dmod = pl->nx;
     {
         void* args[] = {&pl->dp, (void*)&T, (void*)&D, &i_base, &np, &dmod};
-        if ((rc = launch(pl->k4, (unsigned)(pl->nzh * ((pl->nx + KY_NL - 1) / KY_NL)), st, args, "k_ifft_y"))) return rc;
+        if ((rc = launch(pl->k4, (unsigned)(pl->nzh * ((pl->nx + pl->k4.nl - 1) / pl->k4.nl)), st, args, "k_ifft_y"))) return rc;
     }
     if (ev_a) cudaEventRecord(ev_a, st);
     if (pl->fuse56) {
