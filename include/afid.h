@@ -77,6 +77,28 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
  */
 int afid_project(afid_plan* plan, double* u, double* v, double* w, double* p, void* stream);
 
+/*
+ * afid_max_cfl -- SURVEY.md 8(f3): the maximum CFL number of a velocity field, the routine the paper
+ * prints in full (Listing 1 "CalcMaxCFL"):
+ *     cfl = max( 1e-8, max over cells (i,j,k) of
+ *                0.5 * ( |w(i,j,k) + w(i,j,k+1)| / dz + |v(i,j,k) + v(i,j+1,k)| / dy + |u(i,j,k) + u(i+1,j,k)| / dx_i ) )
+ * with periodic wrap in j and k (the listing's dz, dy, udx3m are AFiD's inverse spacings).
+ * u, v, w: DEVICE pointers laid out as for afid_project (read only, 16-byte aligned); cfl: DEVICE pointer to
+ * one double (8-byte aligned), overwritten.  Two kernels are enqueued on `stream`; no host synchronisation.
+ * Typically called on the projected field to pick the next time step.  Returns AFID_OK or a negative code.
+ */
+int afid_max_cfl(afid_plan* plan, const double* u, const double* v, const double* w, double* cfl, void* stream);
+
+/*
+ * afid_plan_set_accumulate -- SURVEY.md 8(f3): choose what afid_project does with p.
+ *   on = 0 (default)  p  = phi   (p is output only; its dx-weighted mean is zero; R6)
+ *   on = 1            p += phi   (the "delta form" pressure update of the fractional step, P:L91, P:L116;
+ *                                 phi then goes through a work array and p is read and written by the
+ *                                 correction kernel: 16 more bytes per point)
+ * The velocity correction is the same in both modes.  Returns AFID_OK or a negative code.
+ */
+int afid_plan_set_accumulate(afid_plan* plan, int on);
+
 /* afid_plan_destroy -- free the plan's device and host memory.  NULL is a no-op.
  * The caller must have synchronised any stream still using the plan. */
 int afid_plan_destroy(afid_plan* plan);

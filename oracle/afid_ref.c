@@ -401,3 +401,36 @@ int afid_ref_project(int nx, int ny, int nz, const double *xc, double Ly, double
     free(d); free(dhat);
     return rc;
 }
+
+/* ------------------------------------------------------------------------------------
+ * the maximum CFL number, the one routine the paper prints in full
+ * (Listing 1 "CalcMaxCFL"):
+ *     cflm = max( 1e-8, max over cells of
+ *                 0.5 * ( |vz(i) + vz(i+1)| * dz + |vy(j) + vy(j+1)| * dy + |vx(k) + vx(k+1)| * udx3m(k) ) )
+ * In AFiD dz, dy and udx3m are INVERSE spacings (R20); in this file's notation
+ * (u wall-normal on x-faces, v, w periodic):
+ *     q(i,j,k) = |w(i,j,k) + w(i,j,k+1)| / dz + |v(i,j,k) + v(i,j+1,k)| / dy + |u(i,j,k) + u(i+1,j,k)| / dx_i
+ * with periodic wrap in j and k.  Plain loops, fp64, the paper's order of operations.
+ * ------------------------------------------------------------------------------------ */
+int afid_ref_max_cfl(int nx, int ny, int nz, const double *xc, double Ly, double Lz,
+                     const double *u, const double *v, const double *w, double *cflm)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || !xc || !u || !v || !w || !cflm) return -1;
+    const double rdy = (double)ny / Ly, rdz = (double)nz / Lz;
+    double best = 0.00000001;
+    for (int i = 0; i < nx; ++i) {
+        const double udx = 1.0 / (xc[i + 1] - xc[i]);
+        for (int j = 0; j < ny; ++j) {
+            const int jp = (j + 1) % ny;
+            for (int k = 0; k < nz; ++k) {
+                const int kp = (k + 1) % nz;
+                const double qcf = fabs((w[IDX(i, j, k)] + w[IDX(i, j, kp)]) * rdz)
+                                 + fabs((v[IDX(i, j, k)] + v[IDX(i, jp, k)]) * rdy)
+                                 + fabs((u[IDX(i, j, k)] + u[IDX(i + 1, j, k)]) * udx);
+                if (qcf * 0.5 > best) best = qcf * 0.5;
+            }
+        }
+    }
+    *cflm = best;
+    return 0;
+}

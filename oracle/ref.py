@@ -128,3 +128,14 @@ def project(xc, Ly, Lz, u, v, w):
                                 C.c_double(Lz), _p(u), _p(v), _p(w), _p(p), C.byref(mi)),
          "afid_ref_project")
     return u, v, w, p, mi.value
+
+
+def max_cfl(xc, Ly, Lz, u, v, w):
+    """Maximum CFL number of the paper's Listing 1, floor 1e-8."""
+    xc, u, v, w = _f64(xc), _f64(u), _f64(v), _f64(w)
+    nx, ny, nz = v.shape
+    assert u.shape == (nx + 1, ny, nz) and w.shape == v.shape and xc.size == nx + 1
+    out = C.c_double(0.0)
+    _chk(lib().afid_ref_max_cfl(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(xc), C.c_double(Ly),
+                                C.c_double(Lz), _p(u), _p(v), _p(w), C.byref(out)), "afid_ref_max_cfl")
+    return out.value

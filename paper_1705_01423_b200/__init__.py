@@ -23,7 +23,7 @@ SYMBOLS = ["afid_plan_create", "afid_project", "afid_plan_destroy", "afid_plan_w
            "afid_plan_num_launches", "afid_stage_forward", "afid_stage_solve", "afid_fft_length_supported",
            "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version",
            "afid_plan_enable_timing", "afid_plan_kernel_times", "afid_plan_kernel_name",
-           "afid_fft_half_length_supported"]
+           "afid_fft_half_length_supported", "afid_max_cfl", "afid_plan_set_accumulate"]
 
 _lib = None
 
@@ -57,6 +57,10 @@ def lib():
         L.afid_stage_forward.argtypes = [vp, vp, vp, vp, vp, vp]
         L.afid_stage_solve.restype = i
         L.afid_stage_solve.argtypes = [vp, vp, vp]
+        L.afid_plan_set_accumulate.restype = i
+        L.afid_plan_set_accumulate.argtypes = [vp, i]
+        L.afid_max_cfl.restype = i
+        L.afid_max_cfl.argtypes = [vp, vp, vp, vp, vp, vp]
         L.afid_fft_length_supported.restype = i
         L.afid_fft_length_supported.argtypes = [i]
         L.afid_fft_half_length_supported.restype = i
@@ -157,6 +161,20 @@ class Plan:
         """afid_stage_solve: in-place x-solves on a [i][kz][ky] spectrum."""
         m = 2 * self.nx * self.nzh * self.ny
         _check(lib().afid_stage_solve(self._h, _dev_ptr(spec, m, "spec"), self._stream(stream)))
+
+    def set_accumulate(self, on=True):
+        """afid_plan_set_accumulate: p += phi instead of p = phi."""
+        _check(lib().afid_plan_set_accumulate(self._h, 1 if on else 0))
+
+    def max_cfl(self, u, v, w, out=None, stream=None):
+        """afid_max_cfl: maximum CFL number (paper's Listing 1) into a 1-element fp64 CUDA tensor (enqueued)."""
+        import torch
+        n = self.nx * self.ny * self.nz
+        if out is None:
+            out = torch.empty(1, dtype=torch.float64, device=u.device)
+        _check(lib().afid_max_cfl(self._h, _dev_ptr(u, n + self.ny * self.nz, "u"), _dev_ptr(v, n, "v"),
+                                  _dev_ptr(w, n, "w"), _dev_ptr(out, 1, "cfl"), self._stream(stream)))
+        return out
 
     def enable_timing(self, on=True):
         """afid_plan_enable_timing: record CUDA events around each kernel of project()."""

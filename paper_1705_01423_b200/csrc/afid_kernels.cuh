@@ -599,8 +599,9 @@ __global__ void __launch_bounds__(LPR* PL::TPL, (LPR * PL::TPL <= 384) ? 2 : 1)
 constexpr int K6_JL = 4, K6_TX = 64, K6_U = 4;
 
 __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const double* __restrict__ p, double* __restrict__ u,
-                                                          double* __restrict__ v, double* __restrict__ w, int i_base, int np)
+                                                          double* __restrict__ v, double* __restrict__ w, int i_base, int np, double* __restrict__ pacc)
 {
+    // `p` holds phi; if pacc != nullptr the pressure is accumulated as well: pacc += phi (P:L91, P:L116 delta form)
     constexpr int JL = K6_JL, TX = K6_TX, U = K6_U;
     // this launch covers planes i_base .. i_base+np-1.
     // CTA order: j-chunks of 32 lines outermost, then i, then the group inside the chunk, so that
@@ -655,6 +656,13 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const dou
                 ww[r].y -= (ph[r].y - ph[r].x) * rdz;
                 stc_h(reinterpret_cast<cplx*>(vl + 2 * kp), vv[r], pol_out);
                 stc_h(reinterpret_cast<cplx*>(wl + 2 * kp), ww[r], pol_out);
+                if (pacc) {
+                    double2* q = reinterpret_cast<double2*>(pacc + ol + 2 * kp);
+                    double2 t = *q;
+                    t.x += ph[r].x;
+                    t.y += ph[r].y;
+                    *q = t;
+                }
                 if (has_u) {
                     uu[r].x -= (ph[r].x - pi[r].x) * rdc;
                     uu[r].y -= (ph[r].y - pi[r].y) * rdc;
@@ -999,6 +1007,75 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
     {   // the mean-mode CTA: contiguous store of the tile
         cplx* dst = T + ((size_t)kz * nkt + ky0 / 8) * (size_t)nx * 8 + (ky0 % 8);
         for (int e = threadIdx.x; e < nx * KW; e += blockDim.x) dst[(e / KW) * 8 + (e % KW)] = tile[e];
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// maximum CFL number, the paper's Listing 1 "CalcMaxCFL":
+//   cflm = max(1e-8, max over cells 0.5 (|w(k)+w(k+1)|/dz + |v(j)+v(j+1)|/dy + |u(i)+u(i+1)|/dx_i))
+// (AFiD's dz, dy, udx3m are inverse spacings).  Same CTA map as K6: (i, 4 lines), four 16-byte pairs per
+// thread per batch; plane i+1 of u and line j+1 of v are L2 hits.  Non-negative doubles order like
+// their bit patterns, so the grid-wide maximum is one atomicMax on the 64-bit pattern per CTA.
+// ------------------------------------------------------------------------------------------
+__global__ void k_cfl_init(double* __restrict__ cfl) { *cfl = 0.00000001; }
+
+__global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const double* __restrict__ u, const double* __restrict__ v,
+                                                          const double* __restrict__ w, double* __restrict__ cfl)
+{
+    constexpr int JL = K6_JL, TX = K6_TX, U = K6_U;
+    __shared__ double s_max[JL * TX / 32];
+    const int ngrp = P.ny / JL;
+    constexpr int JC = 32 / JL;
+    const int per_chunk = P.nx * JC;
+    int i, jg;
+    {
+        const int chunk = blockIdx.x / per_chunk, rem = blockIdx.x % per_chunk;
+        const int jc_here = min(JC, ngrp - chunk * JC);
+        i = rem / jc_here;
+        jg = chunk * JC + rem % jc_here;
+    }
+    const int j = jg * JL + threadIdx.y;
+    const int jp = (j + 1 == P.ny) ? 0 : j + 1;
+    const size_t plane = (size_t)P.ny * P.nz;
+    const size_t ol = ((size_t)i * P.ny + j) * P.nz;
+    const double *ul = u + ol, *vl = v + ol, *wl = w + ol;
+    const double* vp = v + ((size_t)i * P.ny + jp) * P.nz;
+    const int nzh2 = P.nz / 2;
+    const double rdx = __ldg(&P.rdx[i]), rdy = P.rdy, rdz = P.rdz;
+    double best = 0.0;
+    for (int k0 = threadIdx.x; k0 < nzh2; k0 += TX * U) {
+        double2 u0[U], u1[U], v0[U], v1[U], w0[U];
+        double wn[U];
+#pragma unroll
+        for (int r = 0; r < U; ++r) {
+            const int kp = k0 + r * TX;
+            if (kp < nzh2) {
+                u0[r] = ldg2(ul + 2 * kp);
+                u1[r] = ldg2(ul + plane + 2 * kp);
+                v0[r] = ldg2(vl + 2 * kp);
+                v1[r] = ldg2(vp + 2 * kp);
+                w0[r] = ldg2(wl + 2 * kp);
+                wn[r] = __ldg(wl + (kp == nzh2 - 1 ? 0 : 2 * kp + 2));
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < U; ++r) {
+            const int kp = k0 + r * TX;
+            if (kp < nzh2) {
+                const double qa = fabs((w0[r].x + w0[r].y) * rdz) + fabs((v0[r].x + v1[r].x) * rdy) + fabs((u0[r].x + u1[r].x) * rdx);
+                const double qb = fabs((w0[r].y + wn[r]) * rdz) + fabs((v0[r].y + v1[r].y) * rdy) + fabs((u0[r].y + u1[r].y) * rdx);
+                best = fmax(best, fmax(qa, qb) * 0.5);
+            }
+        }
+    }
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, d));
+    const int tid = threadIdx.y * TX + threadIdx.x;
+    if ((tid & 31) == 0) s_max[tid >> 5] = best;
+    __syncthreads();
+    if (tid == 0) {
+        for (int k = 1; k < JL * TX / 32; ++k) best = fmax(best, s_max[k]);
+        atomicMax(reinterpret_cast<unsigned long long*>(cfl), (unsigned long long)__double_as_longlong(best));
     }
 }
 

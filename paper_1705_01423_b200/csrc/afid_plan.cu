@@ -179,6 +179,7 @@ struct afid_plan {
     cplx* ws[2];       // work arrays, nx*nzh*ny complex each
     size_t ws_bytes;
     LaunchCfg k1, k2, k4, k5, k56, k3;
+    bool accumulate;   // p += phi instead of p = phi (afid_plan_set_accumulate)
     bool fuse56;       // K5 and K6 as one kernel (k_c2r_correct) with inter-CTA flags
     unsigned* sync56;  // ticket + one flag per tile (device)
     unsigned epoch;    // call counter: the value the flags of the current call take
@@ -419,9 +420,9 @@ static int run_solve(afid_plan* pl, cplx* outT, cudaStream_t st)
     return launch(pl->k3, (unsigned)(pl->nzh * (pl->ny / pl->k3_kw)), st, args, "k_solve_x");
 }
 
-static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st)
+static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st, double* pacc)
 {
-    void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, &i_base, &np};
+    void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, &i_base, &np, (void*)&pacc};
     cudaError_t e = cudaLaunchKernel((const void*)k_correct, dim3((unsigned)(np * (pl->ny / K6_JL))), dim3(K6_TX, K6_JL), args, 0, st);
     if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_correct: ") + cudaGetErrorString(e));
     return AFID_OK;
@@ -443,12 +444,14 @@ static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double*
         void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&p, (void*)&u, (void*)&v, (void*)&w, (void*)&pl->sync56, &epoch};
         return launch(pl->k56, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_correct");
     }
+    // accumulate mode: phi goes to the (now dead) T work array, K6 corrects from it and adds it to p
+    double* phi = pl->accumulate ? reinterpret_cast<double*>(pl->ws[0]) : p;
     {
-        void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&p, &i_base, &dmod};
+        void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&phi, &i_base, &dmod};
         if ((rc = launch(pl->k5, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_z"))) return rc;
     }
     if (ev_b) cudaEventRecord(ev_b, st);
-    return launch_correct(pl, u, v, w, p, 0, pl->nx, st);
+    return launch_correct(pl, u, v, w, phi, 0, pl->nx, st, pl->accumulate ? p : nullptr);
 }
 
 int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void* stream)
@@ -467,6 +470,29 @@ int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void
     if (tm) cudaEventRecord(pl->ev[3], st);
     if ((rc = run_inverse(pl, pl->ws[0], pl->ws[1], u, v, w, p, st, tm ? pl->ev[4] : nullptr, tm ? pl->ev[5] : nullptr))) return rc;
     if (tm) { cudaEventRecord(pl->ev[6], st); pl->ev_valid = true; }
+    return AFID_OK;
+}
+
+int afid_max_cfl(afid_plan* pl, const double* u, const double* v, const double* w, double* cfl, void* stream)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    int rc;
+    if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w"))) return rc;
+    if (!cfl) return fail(AFID_ERR_NULL, "cfl is NULL");
+    if (((size_t)cfl & 7) != 0) return fail(AFID_ERR_ALIGN, "cfl is not 8-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    k_cfl_init<<<1, 1, 0, st>>>(cfl);
+    void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&cfl};
+    cudaError_t e = cudaLaunchKernel((const void*)k_max_cfl, dim3((unsigned)(pl->nx * (pl->ny / K6_JL))), dim3(K6_TX, K6_JL), args, 0, st);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_max_cfl: ") + cudaGetErrorString(e));
+    return AFID_OK;
+}
+
+int afid_plan_set_accumulate(afid_plan* pl, int on)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    if (on && pl->fuse56) return fail(AFID_ERR_UNSUPPORTED_SIZE, "accumulate is not available on the fused K5/K6 path (AFID_FUSE56=1)");
+    pl->accumulate = on != 0;
     return AFID_OK;
 }
 

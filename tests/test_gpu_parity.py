@@ -103,6 +103,56 @@ def test_fused_c2r_correct_path(ov, monkeypatch):
     assert rel(u2, u1) <= 1e-11 and rel(v2, v1) <= 1e-11 and rel(w2, w1) <= 1e-11
 
 
+@pytest.mark.parametrize("ov", [SHAPES[1], SHAPES[4], SHAPES[7], dict(nx=256, ny=256, nz=256, grid="tanh", s=3.0)],
+                         ids=lambda o: f"{o['nx']}x{o['ny']}x{o['nz']}")
+def test_max_cfl_parity(ov):
+    """afid_max_cfl (paper's Listing 1) against the oracle, on the provisional and on the projected field, and
+    the 1e-8 floor.  Both sides form each cell's value by the same three products and two additions in fp64;
+    the reciprocal spacings are rounded differently (the oracle divides ny/Ly and 1/dx in fp64, the plan
+    rounds 1/(Ly/ny) and 1/dx once from long double), each within one ulp, so the maxima agree to a few ulp:
+    tolerance 2e-15 relative."""
+    cfg = synth.config("C1", **ov)
+    xc = synth.grid_faces(cfg)
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    u, v, w = synth.velocity(cfg, xc)
+    plan = afid.Plan(nx, ny, nz, xc, cfg["Ly"], cfg["Lz"])
+    ud, vd, wd = u.cuda(), v.cuda(), w.cuda()
+    got = float(plan.max_cfl(ud, vd, wd).cpu())
+    want = ref.max_cfl(xc, cfg["Ly"], cfg["Lz"], u.numpy(), v.numpy(), w.numpy())
+    assert abs(got - want) <= 2e-15 * want, (got, want)
+    p = torch.empty_like(vd)
+    plan.project(ud, vd, wd, p)
+    got2 = float(plan.max_cfl(ud, vd, wd).cpu())
+    want2 = ref.max_cfl(xc, cfg["Ly"], cfg["Lz"], ud.cpu().numpy(), vd.cpu().numpy(), wd.cpu().numpy())
+    assert abs(got2 - want2) <= 2e-15 * want2, (got2, want2)
+    z = torch.zeros_like(vd)
+    assert float(plan.max_cfl(torch.zeros_like(ud), z, z).cpu()) == 1e-8
+    plan.destroy()
+
+
+def test_accumulate_mode_parity():
+    """afid_plan_set_accumulate(1): p_out = p_in + phi (P:L91, P:L116 delta form); the velocities as before."""
+    cfg = synth.config("C1", nx=40, ny=64, nz=128, grid="tanh", s=3.0)
+    xc = synth.grid_faces(cfg)
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    u, v, w = synth.velocity(cfg, xc)
+    uo, vo, wo, po, _ = ref.project(xc, cfg["Ly"], cfg["Lz"], u.numpy(), v.numpy(), w.numpy())
+    p_in = torch.from_numpy(np.random.default_rng(3).standard_normal((nx, ny, nz)))
+    plan = afid.Plan(nx, ny, nz, xc, cfg["Ly"], cfg["Lz"])
+    plan.set_accumulate(True)
+    ud, vd, wd, pd = u.cuda(), v.cuda(), w.cuda(), p_in.cuda()
+    plan.project(ud, vd, wd, pd)
+    torch.cuda.synchronize()
+    assert rel(pd.cpu().numpy() - p_in.numpy(), po) <= 1e-11
+    assert rel(ud.cpu().numpy(), uo) <= TOL and rel(vd.cpu().numpy(), vo) <= TOL and rel(wd.cpu().numpy(), wo) <= TOL
+    plan.set_accumulate(False)
+    ud, vd, wd = u.cuda(), v.cuda(), w.cuda()
+    plan.project(ud, vd, wd, pd)
+    torch.cuda.synchronize()
+    assert rel(pd.cpu().numpy(), po) <= TOL
+    plan.destroy()
+
+
 def test_stage_taps_parity():
     """Forward spectrum and x-solve separately (stage boundaries of the paper's step list)."""
     cfg = synth.config("C1", nx=37, ny=48, nz=96, grid="tanh", s=3.0, Ly=1.5, Lz=0.75)
