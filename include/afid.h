@@ -99,6 +99,24 @@ int afid_max_cfl(afid_plan* plan, const double* u, const double* v, const double
  */
 int afid_plan_set_accumulate(afid_plan* plan, int on);
 
+/*
+ * afid_xsolve_* -- batched REAL tridiagonal solves in the wall-normal direction on a field in
+ * physical space, the implicit (Crank-Nicolson) wall-normal viscous step of the time integrator (
+ * "batched tridiagonal solvers").  For every (j,k) column of f[i][j][k] (layout of v, w, p), in place:
+ *     -a_i x_{i-1} + (a_i + c_i + lam_i) x_i - c_i x_{i+1} = f_i ,   i = 0..nx-1   (a_0 and c_{nx-1} are ignored)
+ * i.e. (I - theta L_x) x = r scaled by 1/theta, with L_x x = a_i x_{i-1} - (a_i + c_i) x_i + c_i x_{i+1} and
+ * lam_i = 1/theta (+ the Dirichlet ghost-cell terms in the wall rows).  The paper does not print the
+ * coefficients of its scheme (they are in its Refs [19],[27]), so they are the caller's: HOST arrays of nx
+ * doubles, a_i >= 0, c_i >= 0, lam_i > 0 (an M-matrix: the solve is cancellation-free), copied at create.
+ * afid_xsolve_create is synchronous and returns NULL on failure; afid_xsolve_apply only enqueues one kernel
+ * (the x-solve kernel of afid_project, two neighbouring k columns per complex lane) on `stream`;
+ * f: DEVICE, nx*ny*nz doubles, 16-byte aligned.  The plan must outlive the handle.
+ */
+typedef struct afid_xsolve afid_xsolve;
+afid_xsolve* afid_xsolve_create(afid_plan* plan, const double* a, const double* c, const double* lam);
+int afid_xsolve_apply(afid_xsolve* h, double* f, void* stream);
+int afid_xsolve_destroy(afid_xsolve* h);
+
 /* afid_plan_destroy -- free the plan's device and host memory.  NULL is a no-op.
  * The caller must have synchronised any stream still using the plan. */
 int afid_plan_destroy(afid_plan* plan);

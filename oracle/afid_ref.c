@@ -434,3 +434,46 @@ int afid_ref_max_cfl(int nx, int ny, int nz, const double *xc, double Ly, double
     *cflm = best;
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------
+ * batched real tridiagonal solves in x on a field f[i][j][k], in place -- the
+ * implicit wall-normal step of the time integrator ("batched tridiagonal solvers ...
+ * each thread in a block solves a system").  For every column (j,k):
+ *     -a_i x_{i-1} + (a_i + c_i + lam_i) x_i - c_i x_{i+1} = f_i ,  i = 0..nx-1,  a_0 := 0, c_{nx-1} := 0.
+ * Textbook Thomas algorithm (forward elimination, back substitution) in long double, one column at a time.
+ * ------------------------------------------------------------------------------------ */
+int afid_ref_xsolve(int nx, int ny, int nz, const double *a, const double *c, const double *lam, double *f)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || !a || !c || !lam || !f) return -1;
+    int rc = 0;
+#pragma omp parallel
+    {
+        ld *cp = (ld *)malloc(sizeof(ld) * (size_t)nx);
+        ld *dp = (ld *)malloc(sizeof(ld) * (size_t)nx);
+        if (!cp || !dp) {
+#pragma omp critical
+            rc = -3;
+        } else {
+#pragma omp for collapse(2) schedule(static)
+            for (int j = 0; j < ny; ++j)
+                for (int k = 0; k < nz; ++k) {
+                    for (int i = 0; i < nx; ++i) {
+                        const ld sub = (i == 0) ? 0.0L : -(ld)a[i];
+                        const ld sup = (i == nx - 1) ? 0.0L : -(ld)c[i];
+                        const ld diag = ((i == 0) ? 0.0L : (ld)a[i]) + ((i == nx - 1) ? 0.0L : (ld)c[i]) + (ld)lam[i];
+                        const ld den = (i == 0) ? diag : diag - sub * cp[i - 1];
+                        cp[i] = sup / den;
+                        dp[i] = ((ld)f[IDX(i, j, k)] - ((i == 0) ? 0.0L : sub * dp[i - 1])) / den;
+                    }
+                    ld x = dp[nx - 1];
+                    f[IDX(nx - 1, j, k)] = (double)x;
+                    for (int i = nx - 2; i >= 0; --i) {
+                        x = dp[i] - cp[i] * x;
+                        f[IDX(i, j, k)] = (double)x;
+                    }
+                }
+        }
+        free(cp); free(dp);
+    }
+    return rc;
+}

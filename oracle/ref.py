@@ -139,3 +139,13 @@ def max_cfl(xc, Ly, Lz, u, v, w):
     _chk(lib().afid_ref_max_cfl(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(xc), C.c_double(Ly),
                                 C.c_double(Lz), _p(u), _p(v), _p(w), C.byref(out)), "afid_ref_max_cfl")
     return out.value
+
+
+def xsolve(a, c, lam, f):
+    """Column-wise real tridiagonal solves in x of a field (nx, ny, nz); returns a new array."""
+    a, c, lam = _f64(a), _f64(c), _f64(lam)
+    x = _f64(f).copy()
+    nx, ny, nz = x.shape
+    assert a.size == nx and c.size == nx and lam.size == nx
+    _chk(lib().afid_ref_xsolve(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(a), _p(c), _p(lam), _p(x)), "afid_ref_xsolve")
+    return x

@@ -23,7 +23,8 @@ SYMBOLS = ["afid_plan_create", "afid_project", "afid_plan_destroy", "afid_plan_w
            "afid_plan_num_launches", "afid_stage_forward", "afid_stage_solve", "afid_fft_length_supported",
            "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version",
            "afid_plan_enable_timing", "afid_plan_kernel_times", "afid_plan_kernel_name",
-           "afid_fft_half_length_supported", "afid_max_cfl", "afid_plan_set_accumulate"]
+           "afid_fft_half_length_supported", "afid_max_cfl", "afid_plan_set_accumulate", "afid_xsolve_create", "afid_xsolve_apply",
+           "afid_xsolve_destroy"]
 
 _lib = None
 
@@ -57,6 +58,12 @@ def lib():
         L.afid_stage_forward.argtypes = [vp, vp, vp, vp, vp, vp]
         L.afid_stage_solve.restype = i
         L.afid_stage_solve.argtypes = [vp, vp, vp]
+        L.afid_xsolve_create.restype = vp
+        L.afid_xsolve_create.argtypes = [vp, vp, vp, vp]
+        L.afid_xsolve_apply.restype = i
+        L.afid_xsolve_apply.argtypes = [vp, vp, vp]
+        L.afid_xsolve_destroy.restype = i
+        L.afid_xsolve_destroy.argtypes = [vp]
         L.afid_plan_set_accumulate.restype = i
         L.afid_plan_set_accumulate.argtypes = [vp, i]
         L.afid_max_cfl.restype = i
@@ -162,6 +169,10 @@ class Plan:
         m = 2 * self.nx * self.nzh * self.ny
         _check(lib().afid_stage_solve(self._h, _dev_ptr(spec, m, "spec"), self._stream(stream)))
 
+    def xsolve(self, a, c, lam):
+        """afid_xsolve_create: handle for in-place real tridiagonal solves in x on fields of this plan's shape."""
+        return XSolve(self, a, c, lam)
+
     def set_accumulate(self, on=True):
         """afid_plan_set_accumulate: p += phi instead of p = phi."""
         _check(lib().afid_plan_set_accumulate(self._h, 1 if on else 0))
@@ -190,6 +201,36 @@ class Plan:
     def destroy(self):
         if getattr(self, "_h", None):
             lib().afid_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class XSolve:
+    """afid_xsolve_create / afid_xsolve_apply / afid_xsolve_destroy."""
+
+    def __init__(self, plan, a, c, lam):
+        import numpy as np
+        self.plan = plan
+        arrs = [np.ascontiguousarray(x, dtype=np.float64) for x in (a, c, lam)]
+        if any(x.size != plan.nx for x in arrs):
+            raise ValueError("a, c, lam must hold nx values each")
+        self._h = lib().afid_xsolve_create(plan._h, *[x.ctypes.data_as(C.c_void_p) for x in arrs])
+        if not self._h:
+            raise AfidError(*_last_error())
+
+    def apply(self, f, stream=None):
+        """afid_xsolve_apply: f (nx, ny, nz) fp64 CUDA tensor, solved in place column by column (enqueued)."""
+        n = self.plan.nx * self.plan.ny * self.plan.nz
+        _check(lib().afid_xsolve_apply(self._h, _dev_ptr(f, n, "f"), self.plan._stream(stream)))
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().afid_xsolve_destroy(self._h)
             self._h = None
 
     def __del__(self):

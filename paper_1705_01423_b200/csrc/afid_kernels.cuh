@@ -33,6 +33,7 @@ struct DevParams {
     const double* cc;           // [nx]   c_i = 1/(dx_i dc_{i+1}), c_{nx-1} = 0
     const double* lamy;         // [ny]   modified wavenumbers in y
     const double* lamz;         // [nzh]  modified wavenumbers in z
+    const double* rowlam;       // [nx]   per-row diagonal excess lam_i of the implicit x-solve (k_solve_x MODE 1 only)
     const cplx* tw_y;           // [ny]    exp(-2 pi i k/ny)
     const cplx* tw_zh;          // [nz/2]  exp(-2 pi i k/(nz/2))
     const cplx* tw_z;           // [nz/2+1] exp(-2 pi i k/nz)
@@ -732,7 +733,13 @@ __host__ __device__ constexpr int k3_tile_rows(int nx) { return k3_num_boxes(nx)
 
 // KW = systems (consecutive ky) per CTA: 8 (128-byte rows), or 4 (64-byte rows; half the shared memory, so that
 // two CTAs share an SM and one gathers while the other computes -- used when the 8-wide tile allows only one).
-template <int M, bool EXACT, bool COEF_SMEM, int KW>
+// MODE 0: the Poisson systems of the projection (lam = lamy(ky) + lamz(kz) per system, input C, output T).
+// MODE 1: the same solver on a REAL field f[i][j][k] in place, for the implicit wall-normal
+//   step (I - theta L_x) x = r of the time integrator: every (j,k) column is a system
+//   -a_i x_{i-1} + (a_i + c_i + lam_i) x_i - c_i x_{i+1} = f_i with caller-given a_i, c_i >= 0 and a
+//   per-ROW lam_i > 0 (P.ca, P.cc, P.rowlam); two neighbouring k columns ride as the re/im parts of one
+//   "complex" column (the matrix is real), so KW complex columns = 2 KW reals = 32 KW bytes per row.
+template <int M, bool EXACT, bool COEF_SMEM, int KW, int MODE>
 __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams P, const __grid_constant__ CUtensorMap mapC, cplx* __restrict__ T)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -742,8 +749,12 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
     cplx* tile = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u)); // (offset form keeps the shared state space)
     double* red = reinterpret_cast<double*>(tile + (size_t)k3_tile_rows(nx) * KW); // 2 buffers x 5 arrays x [PCH][KW]
     double2* coef = reinterpret_cast<double2*>(red + 10 * PCH * KW);  // [nx + nx/M + 1] {a_i, c_i}, one pad slot per chunk
-    const int nkt = P.ny / 8, ntile = P.ny / KW;
-    const int kz = blockIdx.x / ntile, ky0 = (blockIdx.x % ntile) * KW;   // first ky of this CTA
+    double* lrow = reinterpret_cast<double*>(coef + k3_coef_slots(nx, M)); // MODE 1: [nx + nx/M + 1] lam_i, same slots
+    // MODE 0: tile = (kz, KW consecutive ky).  MODE 1: tile = (j, KW consecutive complex columns = 2 KW k's);
+    // below "kz" is then j and "ky0" the first complex column along z
+    const int ncol = (MODE == 0) ? P.ny : P.nz / 2;
+    const int nkt = P.ny / 8, ntile = ncol / KW;
+    const int kz = blockIdx.x / ntile, ky0 = (blockIdx.x % ntile) * KW;   // first column of this CTA
     const int s = threadIdx.x % KW, q = threadIdx.x / KW;
     const int slot = q * KW + s, NS = PCH * KW;
 
@@ -757,10 +768,13 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         const int nb = k3_num_boxes(nx), br = k3_box_rows(nx);
         const unsigned long long pol = l2_policy((P.hints & 1) ? 1 : 0);
         mbar_expect_tx(&bar, (uint32_t)(nb * br * KW * sizeof(cplx)));
-        for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * KW, &mapC, ky0 * 2, b * br, kz, &bar, pol);
+        for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * KW, &mapC, ky0 * 2, MODE == 0 ? b * br : kz, MODE == 0 ? kz : b * br, &bar, pol);
     }
     if (COEF_SMEM) {
-        for (int i = threadIdx.x; i < nx; i += blockDim.x) coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
+        for (int i = threadIdx.x; i < nx; i += blockDim.x) {
+            coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
+            if (MODE == 1) lrow[i + i / M] = __ldg(&P.rowlam[i]);
+        }
         __syncthreads();
     }
     mbar_wait(&bar, 0);
@@ -770,8 +784,9 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         if (COEF_SMEM) return cq[i - (int)(threadIdx.x / KW) * M];
         return make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
     };
-    const double lam = __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]);
-    const bool cta_singular = (blockIdx.x == 0);
+    const double lam0 = (MODE == 0) ? __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]) : 0.0;
+    auto lam_at = [&](int i) -> double { return MODE == 0 ? lam0 : (COEF_SMEM ? lrow[i + i / M] : __ldg(&P.rowlam[i])); };
+    const bool cta_singular = (MODE == 0) && (blockIdx.x == 0);
     const int i0 = q * M;
     const int i1 = min(i0 + M, nx) - 1; // interface row of this chunk
     double* bA = red;
@@ -805,7 +820,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
                 const double2 ac = ld_ac(i0 + ru);
                 const double a = ac.x, c = ac.y;
                 const cplx f = (ru >= k) ? tile[(i0 + ru) * KW + s] : F[ru < NF ? ru : 0];
-                const double nh = c * hu, nt = fma(c, tu, lam);
+                const double nh = c * hu, nt = fma(c, tu, lam_at(i0 + ru));
                 const double rr = fast_rcp(a + (nh + nt));
                 hu = nh * rr;
                 tu = nt * rr;
@@ -817,7 +832,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
                 const double a = ac.x, c = ac.y;
                 const cplx f = tile[(i0 + k) * KW + s];
                 if (k < NF && k < (M - 1) / 2) F[k] = f;
-                const double nh = a * hd, nt = fma(a, td, lam);
+                const double nh = a * hd, nt = fma(a, td, lam_at(i0 + k));
                 const double rr = fast_rcp(c + (nh + nt));
                 hd = nh * rr;
                 td = nt * rr;
@@ -838,7 +853,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         const double ab = ld_ac(i1).x;
         const cplx f = tile[i1 * KW + s];
         rA = ab * hd;
-        rL = fma(ab, td, lam);
+        rL = fma(ab, td, lam_at(i1));
         rFr = fma(ab, ydr, f.x);
         rFi = fma(ab, ydi, f.y);
     } else {
@@ -850,7 +865,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
                 if (EXACT || i < i1) {
                     const double2 ac = ld_ac(i);
                     const double a = ac.x, c = ac.y;
-                    const double nh = c * h, nt = fma(c, t, lam);
+                    const double nh = c * h, nt = fma(c, t, lam_at(i));
                     const double rr = fast_rcp(a + (nh + nt));
                     const cplx f = tile[i * KW + s];
                     h = nh * rr;
@@ -874,7 +889,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
             if (EXACT || i < i1) {
                 const double2 ac = ld_ac(i);
                 const double a = ac.x, c = ac.y;
-                const double nh = a * h, nt = fma(a, t, lam);
+                const double nh = a * h, nt = fma(a, t, lam_at(i));
                 const double rr = fast_rcp(c + (nh + nt));
                 const cplx f = tile[i * KW + s];
                 h = nh * rr;
@@ -889,7 +904,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         const double ab = ld_ac(i1).x;
         const cplx f = tile[i1 * KW + s];
         rA = ab * h;
-        rL = fma(ab, t, lam);
+        rL = fma(ab, t, lam_at(i1));
         rFr = fma(ab, yr, f.x);
         rFi = fma(ab, yi, f.y);
     }
@@ -949,9 +964,11 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         // T[kz][kyt][i][8]: the tile is contiguous in global memory.  All CTAs but the one holding the
         // mean mode store x straight from the back substitution (128-byte segments per row; the stores
         // drain while the next CTA of this SM already loads its tile).
-        cplx* dst = T + ((size_t)kz * nkt + ky0 / 8) * (size_t)nx * 8 + (ky0 % 8);
+        // MODE 1: in place, row i of the tile = f[i][j][2 ky0 .. 2 ky0 + 2 KW) (rows a plane apart)
+        cplx* dst = (MODE == 0) ? T + ((size_t)kz * nkt + ky0 / 8) * (size_t)nx * 8 + (ky0 % 8) : T + (size_t)kz * (P.nz / 2) + ky0;
+        const size_t rstride = (MODE == 0) ? 8 : (size_t)P.ny * (P.nz / 2);
         if (!cta_singular) {
-            dst[i1 * 8 + s] = mk(xr, xi);
+            dst[i1 * rstride + s] = mk(xr, xi);
 #pragma unroll
             for (int r = M - 2; r >= 0; --r) {
                 const int i = i0 + r;
@@ -959,7 +976,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
                     const cplx y = tile[i * KW + s];
                     xr = fma(G[r], xr, fma(H[r], elr, y.x));
                     xi = fma(G[r], xi, fma(H[r], eli, y.y));
-                    dst[i * 8 + s] = mk(xr, xi);
+                    dst[i * rstride + s] = mk(xr, xi);
                 }
             }
             return;

@@ -138,6 +138,33 @@ bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5, LaunchCfg* k56)
 
 constexpr int MAX_NX = 1536;
 
+// K3 instantiation, block size and shared memory for nx rows; MODE 0 = Poisson systems, 1 = real field in place
+template <int MODE> LaunchCfg select_k3(int nx, int* kw_out)
+{
+    LaunchCfg c{};
+    int M, kw = 8;
+    if (nx < 64) { M = 4; c.fn = (nx % 4 == 0) ? (const void*)k_solve_x<4, true, true, 8, MODE> : (const void*)k_solve_x<4, false, true, 8, MODE>; }
+    else if (nx <= 1024) {
+        M = 16;
+        // 8-wide tiles if two of them fit an SM, else 4-wide ones (two CTAs per SM: one gathers while the other computes)
+        const size_t smem8 = (size_t)k3_tile_rows(nx) * 8 * sizeof(cplx) + (size_t)10 * ((nx + 15) / 16) * 8 * sizeof(double)
+                             + (size_t)k3_coef_slots(nx, 16) * (sizeof(double2) + sizeof(double)) + 128;
+        if (2 * (smem8 + 1024) > 228 * 1024) kw = 4;
+        if (getenv("AFID_K3_KW")) kw = atoi(getenv("AFID_K3_KW")) == 4 ? 4 : 8;
+        if (kw == 8) c.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 8, MODE> : (const void*)k_solve_x<16, false, true, 8, MODE>;
+        else c.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 4, MODE> : (const void*)k_solve_x<16, false, true, 4, MODE>;
+    }
+    else { M = 32; c.fn = (nx % 32 == 0) ? (const void*)k_solve_x<32, true, false, 8, MODE> : (const void*)k_solve_x<32, false, false, 8, MODE>; }
+    const int pch = (nx + M - 1) / M;
+    c.threads = kw * pch;
+    c.smem = (size_t)k3_tile_rows(nx) * kw * sizeof(cplx) + (size_t)10 * pch * kw * sizeof(double)
+             + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * (sizeof(double2) + sizeof(double)) : 0) + 128;
+    c.ctas_per_sm = 4;
+    c.nl = 0;
+    *kw_out = kw;
+    return c;
+}
+
 // cuTensorMapEncodeTiled through the runtime's driver entry point lookup (no link-time
 // dependency on libcuda, so the library still loads on a machine without a driver)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -243,26 +270,7 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
 
     // ---- K3 configuration
-    int M, pch;
-    int kw = 8;
-    if (nx < 64) { M = 4; pl->k3.fn = (nx % 4 == 0) ? (const void*)k_solve_x<4, true, true, 8> : (const void*)k_solve_x<4, false, true, 8>; }
-    else if (nx <= 1024) {
-        M = 16;
-        // 8-wide tiles if two of them fit an SM, else 4-wide ones (two CTAs per SM: one gathers while the other computes)
-        const size_t smem8 = (size_t)k3_tile_rows(nx) * 8 * sizeof(cplx) + (size_t)10 * ((nx + 15) / 16) * 8 * sizeof(double)
-                             + (size_t)k3_coef_slots(nx, 16) * sizeof(double2) + 128;
-        if (2 * (smem8 + 1024) > 228 * 1024) kw = 4;
-        if (getenv("AFID_K3_KW")) kw = atoi(getenv("AFID_K3_KW")) == 4 ? 4 : 8;
-        if (kw == 8) pl->k3.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 8> : (const void*)k_solve_x<16, false, true, 8>;
-        else pl->k3.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 4> : (const void*)k_solve_x<16, false, true, 4>;
-    }
-    else { M = 32; pl->k3.fn = (nx % 32 == 0) ? (const void*)k_solve_x<32, true, false, 8> : (const void*)k_solve_x<32, false, false, 8>; }
-    pch = (nx + M - 1) / M;
-    pl->k3_kw = kw;
-    pl->k3.threads = kw * pch;
-    pl->k3.smem = (size_t)k3_tile_rows(nx) * kw * sizeof(cplx) + (size_t)10 * pch * kw * sizeof(double)
-                  + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * sizeof(double2) : 0) + 128;
-    pl->k3.ctas_per_sm = 4;
+    pl->k3 = select_k3<0>(nx, &pl->k3_kw);
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -493,6 +501,69 @@ int afid_plan_set_accumulate(afid_plan* pl, int on)
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     if (on && pl->fuse56) return fail(AFID_ERR_UNSUPPORTED_SIZE, "accumulate is not available on the fused K5/K6 path (AFID_FUSE56=1)");
     pl->accumulate = on != 0;
+    return AFID_OK;
+}
+
+// ---- batched real tridiagonal solves in x on a field (implicit wall-normal step) ----------
+struct afid_xsolve {
+    afid_plan* pl;
+    DevParams dp;      // the plan's parameters with ca, cc, rowlam pointing at this object's tables
+    LaunchCfg k;
+    int kw;
+    double* tables;    // device: a[nx], c[nx], lam[nx]
+};
+
+afid_xsolve* afid_xsolve_create(afid_plan* pl, const double* a, const double* c, const double* lam)
+{
+    g_err.clear();
+    g_err_code = 0;
+    if (!pl || !a || !c || !lam) { fail(AFID_ERR_NULL, "plan, a, c or lam is NULL"); return nullptr; }
+    const int nx = pl->nx;
+    for (int i = 0; i < nx; ++i)
+        if (!(a[i] >= 0.0) || !(c[i] >= 0.0) || !(lam[i] > 0.0) || !std::isfinite(a[i]) || !std::isfinite(c[i]) || !std::isfinite(lam[i])) {
+            fail(AFID_ERR_GRID, "afid_xsolve_create needs finite a_i >= 0, c_i >= 0, lam_i > 0 (an M-matrix)");
+            return nullptr;
+        }
+    afid_xsolve* h = new (std::nothrow) afid_xsolve();
+    if (!h) { fail(AFID_ERR_NOMEM, "host allocation failed"); return nullptr; }
+    h->pl = pl;
+    h->k = select_k3<1>(nx, &h->kw);
+    if (set_smem_attr(h->k) != AFID_OK) { delete h; return nullptr; }
+    if (cudaMalloc((void**)&h->tables, 3 * (size_t)nx * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError(); delete h; fail(AFID_ERR_NOMEM, "cudaMalloc(xsolve tables) failed"); return nullptr;
+    }
+    std::vector<double> t(3 * (size_t)nx);
+    for (int i = 0; i < nx; ++i) { t[i] = (i == 0) ? 0.0 : a[i]; t[nx + i] = (i == nx - 1) ? 0.0 : c[i]; t[2 * nx + i] = lam[i]; }
+    if (cudaMemcpy(h->tables, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaFree(h->tables); delete h; fail(AFID_ERR_CUDA, "cudaMemcpy(xsolve tables) failed"); return nullptr;
+    }
+    h->dp = pl->dp;
+    h->dp.ca = h->tables;
+    h->dp.cc = h->tables + nx;
+    h->dp.rowlam = h->tables + 2 * nx;
+    return h;
+}
+
+int afid_xsolve_apply(afid_xsolve* h, double* f, void* stream)
+{
+    if (!h) return fail(AFID_ERR_NULL, "xsolve handle is NULL");
+    int rc;
+    if ((rc = check_ptr(f, "f"))) return rc;
+    const afid_plan* pl = h->pl;
+    alignas(64) CUtensorMap map;
+    if (!make_map3(&map, f, (uint64_t)pl->nz, (uint64_t)pl->ny, (uint64_t)pl->nx, 2 * (uint32_t)h->kw, 1, (uint32_t)k3_box_rows(pl->nx),
+                   CU_TENSOR_MAP_SWIZZLE_NONE))
+        return fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed");
+    cplx* fc = reinterpret_cast<cplx*>(f);
+    void* args[] = {&h->dp, (void*)&map, (void*)&fc};
+    return launch(h->k, (unsigned)(pl->ny * ((pl->nz / 2) / h->kw)), (cudaStream_t)stream, args, "k_solve_x(field)");
+}
+
+int afid_xsolve_destroy(afid_xsolve* h)
+{
+    if (!h) return AFID_OK;
+    cudaFree(h->tables);
+    delete h;
     return AFID_OK;
 }
 

@@ -130,6 +130,38 @@ def test_max_cfl_parity(ov):
     plan.destroy()
 
 
+@pytest.mark.parametrize("shape", [(5, 8, 16), (33, 24, 48), (64, 32, 64), (100, 16, 32), (256, 64, 64), (1030, 8, 32), (1024, 16, 64)],
+                         ids=lambda t: "x".join(map(str, t)))
+def test_xsolve_parity(shape):
+    """afid_xsolve_apply against the oracle's long-double Thomas: every K3 instantiation
+    (nx < 64, <= 1024 with 8- and 4-wide tiles, > 1024; full and ragged chunks), coefficients of an implicit
+    diffusion step on the stretched grid with Dirichlet walls, plus a rough random M-matrix."""
+    nx, ny, nz = shape
+    cfg = synth.config("C1", nx=nx, ny=ny, nz=nz, grid="tanh", s=3.0)
+    xc = synth.grid_faces(cfg)
+    dx, dc = ref.metrics(xc)
+    a = np.zeros(nx); c = np.zeros(nx)
+    a[1:] = 1.0 / (dx[1:] * dc[1:nx]); c[:-1] = 1.0 / (dx[:-1] * dc[1:nx])
+    theta = 1e-3                                           # (I - theta L_x) x = r  <=>  lam = 1/theta
+    lam = np.full(nx, 1.0 / theta)
+    lam[0] += 2.0 / dx[0] ** 2; lam[-1] += 2.0 / dx[-1] ** 2  # Dirichlet walls by ghost cells
+    rng = np.random.default_rng(7)
+    plan = afid.Plan(nx, ny, nz, xc, 1.0, 1.0)
+    for (aa, cc, ll) in ((a, c, lam), (rng.uniform(0.1, 1e4, nx), rng.uniform(0.1, 1e4, nx), rng.uniform(1e-2, 10.0, nx))):
+        f = torch.from_numpy(rng.standard_normal((nx, ny, nz)))
+        want = ref.xsolve(aa, cc, ll, f.numpy())
+        xs = plan.xsolve(aa, cc, ll)
+        fd = f.cuda()
+        xs.apply(fd)
+        torch.cuda.synchronize()
+        assert rel(fd.cpu().numpy(), want) <= 1e-13, rel(fd.cpu().numpy(), want)
+        xs.destroy()
+    with pytest.raises(afid.AfidError) as e:               # not an M-matrix
+        plan.xsolve(a, c, np.zeros(nx))
+    assert e.value.code == -4
+    plan.destroy()
+
+
 def test_accumulate_mode_parity():
     """afid_plan_set_accumulate(1): p_out = p_in + phi (P:L91, P:L116 delta form); the velocities as before."""
     cfg = synth.config("C1", nx=40, ny=64, nz=128, grid="tanh", s=3.0)
