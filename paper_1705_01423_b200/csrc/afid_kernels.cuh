@@ -702,15 +702,13 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const dou
 __device__ __forceinline__ double fast_rcp(double x)
 {
     const int hi = __double2hiint(x), lo = __double2loint(x);
-    // 1.m as a float in [1, 2): the top 23 mantissa bits of x under the exponent of 1.0f
-    const unsigned fb = (__funnelshift_l((unsigned)lo, (unsigned)hi, 3) & 0x007FFFFFu) | 0x3F800000u;
+    const unsigned fb = 0x3F800000u | ((unsigned)(hi & 0xFFFFF) << 3) | ((unsigned)lo >> 29); // 1.m as a float in [1, 2)
     float rf;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"(__uint_as_float(fb)));                 // in (0.5, 1]
     const unsigned rb = __float_as_uint(rf);
-    // back to fp64: (rb >> 3) carries the float's exponent and top mantissa bits at the double's positions;
-    // rebias 127 -> 1023 and subtract x's unbiased exponent: + ((1023 - 127 + 1023) << 20) - (hi & 0xFFF00000)
-    const int rhi = (int)(rb >> 3) + 0x77F00000 - (hi & 0x7FF00000);
-    double r = __hiloint2double(rhi, (int)(rb << 29));
+    const int ex = (hi >> 20) & 0x7FF;
+    const int rexp = (int)(rb >> 23) + (1023 - 127) - (ex - 1023);
+    double r = __hiloint2double((rexp << 20) | (int)((rb >> 3) & 0xFFFFF), (int)(rb << 29));
     double e = fma(-x, r, 1.0);
     r = fma(r, e, r);
     e = fma(-x, r, 1.0);
@@ -781,7 +779,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
     // coefficients {a_i, c_i} of row i; `cq` = slot of the chunk's first row (slot(i) = i + i/M = cq + (i - qM))
     const double2* cq = coef + (size_t)(threadIdx.x / KW) * (M + 1);
     auto ld_ac = [&](int i) -> double2 {
-        if (COEF_SMEM) return cq[i - (int)(threadIdx.x / KW) * M];
+        if (COEF_SMEM) return coef[i + i / M];
         return make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
     };
     const double lam0 = (MODE == 0) ? __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]) : 0.0;

@@ -148,7 +148,7 @@ template <int MODE> LaunchCfg select_k3(int nx, int* kw_out)
         M = 16;
         // 8-wide tiles if two of them fit an SM, else 4-wide ones (two CTAs per SM: one gathers while the other computes)
         const size_t smem8 = (size_t)k3_tile_rows(nx) * 8 * sizeof(cplx) + (size_t)10 * ((nx + 15) / 16) * 8 * sizeof(double)
-                             + (size_t)k3_coef_slots(nx, 16) * (sizeof(double2) + sizeof(double)) + 128;
+                             + (size_t)k3_coef_slots(nx, 16) * (sizeof(double2) + (MODE == 1 ? sizeof(double) : 0)) + 128;
         if (2 * (smem8 + 1024) > 228 * 1024) kw = 4;
         if (getenv("AFID_K3_KW")) kw = atoi(getenv("AFID_K3_KW")) == 4 ? 4 : 8;
         if (kw == 8) c.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 8, MODE> : (const void*)k_solve_x<16, false, true, 8, MODE>;
@@ -158,7 +158,7 @@ template <int MODE> LaunchCfg select_k3(int nx, int* kw_out)
     const int pch = (nx + M - 1) / M;
     c.threads = kw * pch;
     c.smem = (size_t)k3_tile_rows(nx) * kw * sizeof(cplx) + (size_t)10 * pch * kw * sizeof(double)
-             + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * (sizeof(double2) + sizeof(double)) : 0) + 128;
+             + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * (sizeof(double2) + (MODE == 1 ? sizeof(double) : 0)) : 0) + 128;
     c.ctas_per_sm = 4;
     c.nl = 0;
     *kw_out = kw;
