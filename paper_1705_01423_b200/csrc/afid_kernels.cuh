@@ -369,22 +369,19 @@ __global__ void __launch_bounds__(LPR* PL::TPL, (LPR * PL::TPL <= 384) ? 2 : 1) 
     }
     auto at = [sm](int l, int r) -> cplx& { return sm[(r << 3) + (l ^ (r & 7))]; };
     mbar_wait(&bar, 0);
-    for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NT) {
-        const int k = idx >> 3, l = idx & 7;
-        const int km = Nh - k;
+    // Hermitian pre-processing fused into the first pass's loads: element e of the complex line is
+    //   Z'(e) = (X(e) + conj X(Nh-e)) + i conj(w^e) (X(e) - conj X(Nh-e)),   w = exp(-2 pi i / nz),
+    // formed from rows k = min(e, Nh-e) and Nh-k (stored re/im-swapped: the inverse runs as a forward transform)
+    auto zprime = [&](int l, int e) -> cplx {
+        const int k = min(e, Nh - e), km = Nh - k;
         const cplx xk = at(l, k);
         const cplx xm = at(l, km);
         const cplx wk = __ldg(&P.tw_z[k]);
-        // E = X(k) + conj X(Nh-k), O = X(k) - conj X(Nh-k)
         const cplx E = mk(xk.x + xm.x, xk.y - xm.y), O = mk(xk.x - xm.x, xk.y + xm.y);
         const cplx wo = mk(fma(wk.y, O.y, wk.x * O.x), fma(-wk.y, O.x, wk.x * O.y)); // conj(w) * O
         const cplx t = mk(-wo.y, wo.x);                                              // i conj(w) O
-        // stored re/im-swapped: the inverse transform runs as a forward one on swapped data
-        at(l, k) = mk(E.y + t.y, E.x + t.x);
-        // Z'(Nh-k) = conj( E - i conj(w) O )
-        if (k != 0 && k != km) at(l, km) = mk(-(E.y - t.y), E.x - t.x);
-    }
-    __syncthreads();
+        return (e == k) ? mk(E.y + t.y, E.x + t.x) : mk(-(E.y - t.y), E.x - t.x);
+    };
     const int lr = threadIdx.x / TPL, tl = threadIdx.x % TPL;
 #pragma unroll 1
     for (int rnd = 0; rnd < NL / LPR; ++rnd) {
@@ -395,7 +392,7 @@ __global__ void __launch_bounds__(LPR* PL::TPL, (LPR * PL::TPL <= 384) ? 2 : 1) 
         typedef FftPass<PL, 0> P0;
         {
             typename P0::Regs rg;
-            P0::load(rg, tl, [&](int e) { return at(ln, e); });   // unpadded rows, as TMA delivered them
+            P0::load(rg, tl, [&](int e) { return zprime(ln, e); });   // unpadded rows, as TMA delivered them
             if constexpr (PL::NPASS == 1) {
                 P0::compute_store(rg, tl, P.tw_zh, st_p);
             } else {
