@@ -152,10 +152,10 @@ template <int R0_, int R1_, int R2_, int R3_, int TPL_> struct FftPlan {
     static constexpr int N = R0 * R1 * R2 * R3;
     static constexpr int NPASS = R1 == 1 ? 1 : (R2 == 1 ? 2 : (R3 == 1 ? 3 : 4));
     // Shared-memory layout of a line: one pad element after every R0 elements, so that the
-    // first pass's stride-R0 writes are bank-conflict free; line stride odd (in 16-byte
-    // units) so that 8 lines accessed at the same offset hit 8 different bank groups.
+    // first pass's stride-R0 writes are bank-conflict free; line stride = 2 mod 8 (in 16-byte
+    // units) so that K1's split pass, whose 8-lane phases touch slots k, k+1 of 4 lines, is too.
     static constexpr int PADDED = N + N / R0; // = pad(N): one extra slot (index N) is kept for K5's Nyquist entry
-    static constexpr int LS = (PADDED % 2 == 0) ? PADDED + 1 : PADDED + 2;
+    static constexpr int LS = PADDED + ((2 - PADDED % 8) + 8) % 8 + ((PADDED % 8 == 2) ? 8 : 0); // = 2 mod 8, > PADDED
     static __device__ __forceinline__ int pad(int e) { return e + e / R0; }
     template <int P> static constexpr int radix() { return P == 0 ? R0 : (P == 1 ? R1 : (P == 2 ? R2 : R3)); }
     template <int P> static constexpr int stride() { return P == 0 ? 1 : (P == 1 ? R0 : (P == 2 ? R0 * R1 : R0 * R1 * R2)); }
