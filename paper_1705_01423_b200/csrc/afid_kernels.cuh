@@ -780,7 +780,11 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         return make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
     };
     const double lam0 = (MODE == 0) ? __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]) : 0.0;
-    auto lam_at = [&](int i) -> double { return MODE == 0 ? lam0 : (COEF_SMEM ? lrow[i + i / M] : __ldg(&P.rowlam[i])); };
+    auto lam_at = [&](int i) -> double {
+        if constexpr (MODE == 0) return lam0;
+        else if constexpr (COEF_SMEM) return lrow[i + i / M];
+        else return __ldg(&P.rowlam[i]);
+    };
     const bool cta_singular = (MODE == 0) && (blockIdx.x == 0);
     const int i0 = q * M;
     const int i1 = min(i0 + M, nx) - 1; // interface row of this chunk
