@@ -50,7 +50,7 @@ typedef struct afid_plan afid_plan; /* opaque; owned by the library */
  *   nx      cells in x, 2 <= nx <= afid_max_nx()
  *   ny, nz  periodic cells; ny and nz/2 must be lengths the FFT kernels are instantiated
  *           for (afid_fft_length_supported, afid_fft_half_length_supported): powers of two
- *           times 1 or 3, ny in 8..4096, nz/2 in 8..1024
+ *           times 1 or 3 (ny in 8..4096, nz/2 in 8..1024), or times 5 (ny in 40..2560, nz/2 in 40..640)
  *   xc      HOST pointer, nx+1 face coordinates (copied; caller keeps ownership)
  *   Ly, Lz  periodic box lengths (> 0)
  * The plan owns: reciprocal metrics, tridiagonal coefficients a_i, c_i, modified

@@ -47,7 +47,14 @@ int fail(int code, const std::string& msg)
     X(1536, 16, 16, 6, 1, 96)   \
     X(2048, 16, 16, 8, 1, 128)  \
     X(3072, 16, 16, 12, 1, 192) \
-    X(4096, 16, 16, 16, 1, 256)
+    X(4096, 16, 16, 16, 1, 256) \
+    X(40, 8, 5, 1, 1, 5)        \
+    X(80, 16, 5, 1, 1, 5)       \
+    X(160, 8, 4, 5, 1, 20)      \
+    X(320, 8, 8, 5, 1, 40)      \
+    X(640, 16, 8, 5, 1, 40)     \
+    X(1280, 16, 16, 5, 1, 80)   \
+    X(2560, 16, 16, 2, 5, 160)
 
 // z-direction lines (K1, K5; complex length nz/2): plans with <= 12 elements per thread where
 // it matters, so that twice as many warps are resident while the loads are in flight
@@ -65,7 +72,12 @@ int fail(int code, const std::string& msg)
     X(384, 8, 8, 6, 1, 48)      \
     X(512, 8, 8, 8, 1, 64)      \
     X(768, 16, 16, 3, 1, 48)    \
-    X(1024, 8, 16, 8, 1, 128)
+    X(1024, 8, 16, 8, 1, 128)   \
+    X(40, 8, 5, 1, 1, 5)        \
+    X(80, 16, 5, 1, 1, 5)       \
+    X(160, 8, 4, 5, 1, 20)      \
+    X(320, 8, 8, 5, 1, 40)      \
+    X(640, 16, 8, 5, 1, 40)
 
 constexpr int K1_NL = 4; // lines per CTA in K1 (two CTAs fill one 128-byte row of B)
 constexpr int K5_LPR = 4; // lines per round in K5 (8 lines per CTA, 2 rounds)

@@ -93,6 +93,23 @@ template <> struct Dft<3> {
         v[2] = mk(t2.x - t3.y, t2.y + t3.x); // t2 + i t3
     }
 };
+template <> struct Dft<5> { // lengths 5 * 2^a (the paper's 1280-point direction, Table 3)
+    static __device__ __forceinline__ void run(cplx (&v)[5])
+    {
+        const double c1 = 0.30901699437494742410, c2 = -0.80901699437494742410; // cos(2 pi/5), cos(4 pi/5)
+        const double s1 = 0.95105651629515357212, s2 = 0.58778525229247312917;  // sin(2 pi/5), sin(4 pi/5)
+        const cplx a1 = cadd(v[1], v[4]), a2 = cadd(v[2], v[3]), b1 = csub(v[1], v[4]), b2 = csub(v[2], v[3]);
+        const cplx r1 = mk(fma(c2, a2.x, fma(c1, a1.x, v[0].x)), fma(c2, a2.y, fma(c1, a1.y, v[0].y)));
+        const cplx r2 = mk(fma(c1, a2.x, fma(c2, a1.x, v[0].x)), fma(c1, a2.y, fma(c2, a1.y, v[0].y)));
+        const cplx i1 = mk(fma(s2, b2.x, s1 * b1.x), fma(s2, b2.y, s1 * b1.y));
+        const cplx i2 = mk(fma(-s1, b2.x, s2 * b1.x), fma(-s1, b2.y, s2 * b1.y));
+        v[0] = cadd(v[0], cadd(a1, a2));
+        v[1] = mk(r1.x + i1.y, r1.y - i1.x); // r1 - i i1
+        v[4] = mk(r1.x - i1.y, r1.y + i1.x); // r1 + i i1
+        v[2] = mk(r2.x + i2.y, r2.y - i2.x); // r2 - i i2
+        v[3] = mk(r2.x - i2.y, r2.y + i2.x); // r2 + i i2
+    }
+};
 template <> struct Dft<4> {
     static __device__ __forceinline__ void run(cplx (&v)[4])
     {

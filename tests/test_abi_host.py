@@ -48,10 +48,14 @@ def test_library_is_sm100a_only(built_lib):
 
 def test_supported_sizes_host_queries(built_lib):
     import paper_1705_01423_b200 as afid
-    for n in (16, 32, 128, 256, 512, 768, 1024, 1536, 4096):
+    for n in (16, 32, 128, 256, 512, 768, 1024, 1536, 4096, 40, 320, 1280, 2560):
         assert afid.fft_length_supported(n), n
-    for n in (0, 7, 15, 40, 100, 1000, 5000):
+    for n in (0, 7, 15, 20, 100, 1000, 5000, 3200):
         assert not afid.fft_length_supported(n), n
+    for n in (8, 768, 1024, 40, 640):
+        assert afid.fft_half_length_supported(n), n
+    for n in (1280, 1536, 50):
+        assert not afid.fft_half_length_supported(n), n
     assert afid.max_nx() >= 1024
 
 
@@ -66,7 +70,7 @@ def test_no_cpu_fallback_without_device(built_lib):
     assert e.value.code == -6
     # argument validation happens before the device is touched
     with pytest.raises(afid.AfidError) as e:
-        afid.Plan(32, 40, 32, np.linspace(0.0, 1.0, 33), 1.0, 1.0)
+        afid.Plan(32, 56, 32, np.linspace(0.0, 1.0, 33), 1.0, 1.0)
     assert e.value.code == -3
 
 

@@ -78,6 +78,14 @@ SHAPES = [
     dict(nx=40, ny=64, nz=128, grid="tanh", s=3.0, M=32, expo=-5.0 / 6.0),
     dict(nx=17, ny=128, nz=256, grid="uniform"),
     dict(nx=16, ny=384, nz=192, grid="tanh", s=3.0),
+    # lengths 5 * 2^a (radix-5 passes), every such plan at least once in y and in z
+    dict(nx=6, ny=40, nz=80, grid="tanh", s=3.0, Ly=1.3),
+    dict(nx=9, ny=160, nz=320, grid="tanh", s=3.0),
+    dict(nx=4, ny=80, nz=1280, grid="uniform", Lz=2.5),
+    dict(nx=3, ny=640, nz=160, grid="tanh", s=3.0),
+    dict(nx=2, ny=1280, nz=640, grid="uniform"),
+    dict(nx=2, ny=2560, nz=80, grid="tanh", s=3.0),
+    dict(nx=5, ny=320, nz=80, grid="tanh", s=3.0),
 ]
 
 
@@ -235,7 +243,7 @@ def test_c2_full_parity():
 def test_error_codes():
     xc = np.linspace(0.0, 1.0, 33)
     with pytest.raises(afid.AfidError) as e:
-        afid.Plan(32, 40, 32, xc, 1.0, 1.0)           # 40 is not a supported FFT length
+        afid.Plan(32, 56, 32, xc, 1.0, 1.0)           # 56 = 7 * 8 is not a supported FFT length
     assert e.value.code == -3
     with pytest.raises(afid.AfidError) as e:
         afid.Plan(32, 32, 30, xc, 1.0, 1.0)           # nz/2 = 15
