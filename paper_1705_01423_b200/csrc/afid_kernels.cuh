@@ -33,7 +33,6 @@ struct DevParams {
     const double* cc;           // [nx]   c_i = 1/(dx_i dc_{i+1}), c_{nx-1} = 0
     const double* lamy;         // [ny]   modified wavenumbers in y
     const double* lamz;         // [nzh]  modified wavenumbers in z
-    const double* rowlam;       // [nx]   per-row diagonal excess lam_i of the implicit x-solve (k_solve_x MODE 1 only)
     const cplx* tw_y;           // [ny]    exp(-2 pi i k/ny)
     const cplx* tw_zh;          // [nz/2]  exp(-2 pi i k/(nz/2))
     const cplx* tw_z;           // [nz/2+1] exp(-2 pi i k/nz)
@@ -728,13 +727,7 @@ __host__ __device__ constexpr int k3_tile_rows(int nx) { return k3_num_boxes(nx)
 
 // KW = systems (consecutive ky) per CTA: 8 (128-byte rows), or 4 (64-byte rows; half the shared memory, so that
 // two CTAs share an SM and one gathers while the other computes -- used when the 8-wide tile allows only one).
-// MODE 0: the Poisson systems of the projection (lam = lamy(ky) + lamz(kz) per system, input C, output T).
-// MODE 1: the same solver on a REAL field f[i][j][k] in place, for the implicit wall-normal
-//   step (I - theta L_x) x = r of the time integrator: every (j,k) column is a system
-//   -a_i x_{i-1} + (a_i + c_i + lam_i) x_i - c_i x_{i+1} = f_i with caller-given a_i, c_i >= 0 and a
-//   per-ROW lam_i > 0 (P.ca, P.cc, P.rowlam); two neighbouring k columns ride as the re/im parts of one
-//   "complex" column (the matrix is real), so KW complex columns = 2 KW reals = 32 KW bytes per row.
-template <int M, bool EXACT, bool COEF_SMEM, int KW, int MODE>
+template <int M, bool EXACT, bool COEF_SMEM, int KW>
 __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams P, const __grid_constant__ CUtensorMap mapC, cplx* __restrict__ T)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -744,12 +737,8 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
     cplx* tile = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u)); // (offset form keeps the shared state space)
     double* red = reinterpret_cast<double*>(tile + (size_t)k3_tile_rows(nx) * KW); // 2 buffers x 5 arrays x [PCH][KW]
     double2* coef = reinterpret_cast<double2*>(red + 10 * PCH * KW);  // [nx + nx/M + 1] {a_i, c_i}, one pad slot per chunk
-    double* lrow = reinterpret_cast<double*>(coef + k3_coef_slots(nx, M)); // MODE 1: [nx + nx/M + 1] lam_i, same slots
-    // MODE 0: tile = (kz, KW consecutive ky).  MODE 1: tile = (j, KW consecutive complex columns = 2 KW k's);
-    // below "kz" is then j and "ky0" the first complex column along z
-    const int ncol = (MODE == 0) ? P.ny : P.nz / 2;
-    const int nkt = P.ny / 8, ntile = ncol / KW;
-    const int kz = blockIdx.x / ntile, ky0 = (blockIdx.x % ntile) * KW;   // first column of this CTA
+    const int nkt = P.ny / 8, ntile = P.ny / KW;
+    const int kz = blockIdx.x / ntile, ky0 = (blockIdx.x % ntile) * KW;   // first ky of this CTA
     const int s = threadIdx.x % KW, q = threadIdx.x / KW;
     const int slot = q * KW + s, NS = PCH * KW;
 
@@ -763,13 +752,10 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         const int nb = k3_num_boxes(nx), br = k3_box_rows(nx);
         const unsigned long long pol = l2_policy((P.hints & 1) ? 1 : 0);
         mbar_expect_tx(&bar, (uint32_t)(nb * br * KW * sizeof(cplx)));
-        for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * KW, &mapC, ky0 * 2, MODE == 0 ? b * br : kz, MODE == 0 ? kz : b * br, &bar, pol);
+        for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * KW, &mapC, ky0 * 2, b * br, kz, &bar, pol);
     }
     if (COEF_SMEM) {
-        for (int i = threadIdx.x; i < nx; i += blockDim.x) {
-            coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
-            if (MODE == 1) lrow[i + i / M] = __ldg(&P.rowlam[i]);
-        }
+        for (int i = threadIdx.x; i < nx; i += blockDim.x) coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
         __syncthreads();
     }
     mbar_wait(&bar, 0);
@@ -779,13 +765,8 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         if (COEF_SMEM) return coef[i + i / M];
         return make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
     };
-    const double lam0 = (MODE == 0) ? __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]) : 0.0;
-    auto lam_at = [&](int i) -> double {
-        if constexpr (MODE == 0) return lam0;
-        else if constexpr (COEF_SMEM) return lrow[i + i / M];
-        else return __ldg(&P.rowlam[i]);
-    };
-    const bool cta_singular = (MODE == 0) && (blockIdx.x == 0);
+    const double lam = __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]);
+    const bool cta_singular = (blockIdx.x == 0);
     const int i0 = q * M;
     const int i1 = min(i0 + M, nx) - 1; // interface row of this chunk
     double* bA = red;
@@ -819,7 +800,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
                 const double2 ac = ld_ac(i0 + ru);
                 const double a = ac.x, c = ac.y;
                 const cplx f = (ru >= k) ? tile[(i0 + ru) * KW + s] : F[ru < NF ? ru : 0];
-                const double nh = c * hu, nt = fma(c, tu, lam_at(i0 + ru));
+                const double nh = c * hu, nt = fma(c, tu, lam);
                 const double rr = fast_rcp(a + (nh + nt));
                 hu = nh * rr;
                 tu = nt * rr;
@@ -831,7 +812,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
                 const double a = ac.x, c = ac.y;
                 const cplx f = tile[(i0 + k) * KW + s];
                 if (k < NF && k < (M - 1) / 2) F[k] = f;
-                const double nh = a * hd, nt = fma(a, td, lam_at(i0 + k));
+                const double nh = a * hd, nt = fma(a, td, lam);
                 const double rr = fast_rcp(c + (nh + nt));
                 hd = nh * rr;
                 td = nt * rr;
@@ -852,7 +833,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         const double ab = ld_ac(i1).x;
         const cplx f = tile[i1 * KW + s];
         rA = ab * hd;
-        rL = fma(ab, td, lam_at(i1));
+        rL = fma(ab, td, lam);
         rFr = fma(ab, ydr, f.x);
         rFi = fma(ab, ydi, f.y);
     } else {
@@ -864,7 +845,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
                 if (EXACT || i < i1) {
                     const double2 ac = ld_ac(i);
                     const double a = ac.x, c = ac.y;
-                    const double nh = c * h, nt = fma(c, t, lam_at(i));
+                    const double nh = c * h, nt = fma(c, t, lam);
                     const double rr = fast_rcp(a + (nh + nt));
                     const cplx f = tile[i * KW + s];
                     h = nh * rr;
@@ -888,7 +869,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
             if (EXACT || i < i1) {
                 const double2 ac = ld_ac(i);
                 const double a = ac.x, c = ac.y;
-                const double nh = a * h, nt = fma(a, t, lam_at(i));
+                const double nh = a * h, nt = fma(a, t, lam);
                 const double rr = fast_rcp(c + (nh + nt));
                 const cplx f = tile[i * KW + s];
                 h = nh * rr;
@@ -903,7 +884,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         const double ab = ld_ac(i1).x;
         const cplx f = tile[i1 * KW + s];
         rA = ab * h;
-        rL = fma(ab, t, lam_at(i1));
+        rL = fma(ab, t, lam);
         rFr = fma(ab, yr, f.x);
         rFi = fma(ab, yi, f.y);
     }
@@ -963,9 +944,8 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         // T[kz][kyt][i][8]: the tile is contiguous in global memory.  All CTAs but the one holding the
         // mean mode store x straight from the back substitution (128-byte segments per row; the stores
         // drain while the next CTA of this SM already loads its tile).
-        // MODE 1: in place, row i of the tile = f[i][j][2 ky0 .. 2 ky0 + 2 KW) (rows a plane apart)
-        cplx* dst = (MODE == 0) ? T + ((size_t)kz * nkt + ky0 / 8) * (size_t)nx * 8 + (ky0 % 8) : T + (size_t)kz * (P.nz / 2) + ky0;
-        const size_t rstride = (MODE == 0) ? 8 : (size_t)P.ny * (P.nz / 2);
+        cplx* dst = T + ((size_t)kz * nkt + ky0 / 8) * (size_t)nx * 8 + (ky0 % 8);
+        constexpr int rstride = 8;
         if (!cta_singular) {
             dst[i1 * rstride + s] = mk(xr, xi);
 #pragma unroll
@@ -1023,6 +1003,129 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
     {   // the mean-mode CTA: contiguous store of the tile
         cplx* dst = T + ((size_t)kz * nkt + ky0 / 8) * (size_t)nx * 8 + (ky0 % 8);
         for (int e = threadIdx.x; e < nx * KW; e += blockDim.x) dst[(e / KW) * 8 + (e % KW)] = tile[e];
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// SURVEY.md 8(f1), fast path: the x-solve of a REAL field when every column has the SAME matrix (the implicit
+// wall-normal step): all pivot quantities of k_solve_x's algorithm (two-sided chunk elimination, reduced
+// interface system, PCR, back substitution) depend only on the row, so afid_xsolve_create evaluates them once
+// on the host in long double and the kernel only runs the data recurrences:
+//   up    yu <- (c rr)_i yu + (rr)_i f_i                 (UP[i]  = {c_i rr_i, rr_i},  rows i1-1 .. i0)
+//   down  yd <- (a rr)_i yd + (rr)_i f_i ,  tile <- yd   (DN[i]  = {a_i rr_i, rr_i},  rows i0 .. i1-1)
+//   F_q   = f_i1 + ab_q yd + cb_{q+1} yu_{q+1}           (CH[q]  = {ab_q, cb_q})
+//   PCR   F_q <- F_q + al F_{q-d} + ga F_{q+d}           (PC[lev][q] = {al, ga}),  E_q = rrE_q F_q
+//   back  x_i = y_i + G_i x_{i+1} + H_i E_{q-1}          (GH[i]  = {G_i, H_i})
+// Tile = (line j, KW complex lanes = 2 KW real k columns) x all nx rows, rows a plane apart, gathered by TMA;
+// thread (s, q) owns rows [qM, qM+M) of lane s, as in k_solve_x.  KW = 8 (128-byte rows) wherever the tile
+// fits: 64-byte rows a plane apart run at 0.43 of the copy bandwidth, 128-byte rows at 0.5-0.63 (an L2
+// prefetch of the full lines before the 64-byte gather made it slower).  The tables are read through L1.
+// ------------------------------------------------------------------------------------------
+struct XsTables {
+    const double2* UP;   // [nx]
+    const double2* DN;   // [nx]
+    const double2* GH;   // [nx]
+    const double2* CH;   // [PCH]  {ab_q, cb_q}
+    const double* RE;    // [PCH]  1 / (A + C + L) of the fully reduced row
+    const double2* PC;   // [nlev][PCH] {al, ga}
+    int nlev;
+};
+
+template <int M, int KW>
+__global__ void __launch_bounds__(64 * KW, (KW == 4) ? 3 : 1) k_xsolve_field(DevParams P, XsTables X, const __grid_constant__ CUtensorMap map, cplx* __restrict__ F)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bar;
+    const int nx = P.nx, PCH = blockDim.x / KW;
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u));   // [k3_tile_rows(nx)][KW]
+    cplx* red = tile + (size_t)k3_tile_rows(nx) * KW;                                                  // 2 x [PCH][KW]
+    const int ntile = (P.nz / 2) / KW;
+    const int j = blockIdx.x / ntile, c0 = (blockIdx.x % ntile) * KW;   // line j, first complex column
+    const int s = threadIdx.x % KW, q = threadIdx.x / KW;
+    const int slot = q * KW + s, NS = PCH * KW;
+    if (threadIdx.x == 0) {
+        mbar_init(&bar, 1);
+        fence_mbar_init();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int nb = k3_num_boxes(nx), br = k3_box_rows(nx);
+        const unsigned long long pol = l2_policy((P.hints & 1) ? 1 : 0);
+        mbar_expect_tx(&bar, (uint32_t)(nb * br * KW * sizeof(cplx)));
+        for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * KW, &map, c0 * 2, j, b * br, &bar, pol);
+    }
+    const int i0 = q * M;
+    const int i1 = min(i0 + M, nx) - 1; // interface row of this chunk
+    const double2 ch = __ldg(&X.CH[q]);
+    mbar_wait(&bar, 0);
+    cplx* my = tile + (size_t)i0 * KW + s;
+    // upward: relation of the first interior row to the interface above (read only)
+    double ur = 0.0, ui = 0.0;
+#pragma unroll
+    for (int r = M - 2; r >= 0; --r) {
+        if (i0 + r < i1) {
+            const double2 t = __ldg(&X.UP[i0 + r]);
+            const cplx f = my[r * KW];
+            ur = fma(t.x, ur, t.y * f.x);
+            ui = fma(t.x, ui, t.y * f.y);
+        }
+    }
+    if (q > 0) red[NS + slot - KW] = mk(ch.y * ur, ch.y * ui); // cb_q yu_q -> reduced row q-1 (staged in buffer 1)
+    // downward, in place: tile <- y
+    double dr = 0.0, di = 0.0;
+#pragma unroll
+    for (int r = 0; r < M - 1; ++r) {
+        if (i0 + r < i1) {
+            const double2 t = __ldg(&X.DN[i0 + r]);
+            const cplx f = my[r * KW];
+            dr = fma(t.x, dr, t.y * f.x);
+            di = fma(t.x, di, t.y * f.y);
+            my[r * KW] = mk(dr, di);
+        }
+    }
+    double fr, fi;
+    {
+        const cplx f = tile[(size_t)i1 * KW + s];
+        fr = fma(ch.x, dr, f.x);
+        fi = fma(ch.x, di, f.y);
+    }
+    __syncthreads();
+    if (q < PCH - 1) {
+        const cplx t = red[NS + slot];
+        fr += t.x;
+        fi += t.y;
+    }
+    // PCR on the right-hand side only (the matrix part was done on the host)
+    cplx* bA = red;
+    cplx* bB = red + NS;
+    for (int lev = 0, d = 1; lev < X.nlev; ++lev, d <<= 1) {
+        __syncthreads();            // previous level's reads (and the staging reads above) are done
+        bA[slot] = mk(fr, fi);
+        __syncthreads();
+        const double2 pc = __ldg(&X.PC[lev * PCH + q]);
+        if (q - d >= 0) { const cplx m = bA[slot - KW * d]; fr = fma(pc.x, m.x, fr); fi = fma(pc.x, m.y, fi); }
+        if (q + d < PCH) { const cplx m = bA[slot + KW * d]; fr = fma(pc.y, m.x, fr); fi = fma(pc.y, m.y, fi); }
+        cplx* tp = bA; bA = bB; bB = tp;
+    }
+    const double re = __ldg(&X.RE[q]);
+    double xr = fr * re, xi = fi * re;
+    __syncthreads();
+    bA[slot] = mk(xr, xi);
+    __syncthreads();
+    const cplx el = (q > 0) ? bA[slot - KW] : mk(0.0, 0.0);
+    // back substitution with direct stores: row i of the tile = F[i][j][2 c0 .. 2 c0 + 2 KW)
+    cplx* dst = F + (size_t)j * (P.nz / 2) + c0 + s;
+    const size_t rstride = (size_t)P.ny * (P.nz / 2);
+    dst[(size_t)i1 * rstride] = mk(xr, xi);
+#pragma unroll
+    for (int r = M - 2; r >= 0; --r) {
+        if (i0 + r < i1) {
+            const double2 gh = __ldg(&X.GH[i0 + r]);
+            const cplx y = my[r * KW];
+            xr = fma(gh.x, xr, fma(gh.y, el.x, y.x));
+            xi = fma(gh.x, xi, fma(gh.y, el.y, y.y));
+            dst[(size_t)(i0 + r) * rstride] = mk(xr, xi);
+        }
     }
 }
 

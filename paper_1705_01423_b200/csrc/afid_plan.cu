@@ -150,27 +150,27 @@ bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5, LaunchCfg* k56)
 
 constexpr int MAX_NX = 1536;
 
-// K3 instantiation, block size and shared memory for nx rows; MODE 0 = Poisson systems, 1 = real field in place
-template <int MODE> LaunchCfg select_k3(int nx, int* kw_out)
+// K3 instantiation, block size and shared memory for nx rows
+LaunchCfg select_k3(int nx, int* kw_out)
 {
     LaunchCfg c{};
     int M, kw = 8;
-    if (nx < 64) { M = 4; c.fn = (nx % 4 == 0) ? (const void*)k_solve_x<4, true, true, 8, MODE> : (const void*)k_solve_x<4, false, true, 8, MODE>; }
+    if (nx < 64) { M = 4; c.fn = (nx % 4 == 0) ? (const void*)k_solve_x<4, true, true, 8 > : (const void*)k_solve_x<4, false, true, 8 >; }
     else if (nx <= 1024) {
         M = 16;
         // 8-wide tiles if two of them fit an SM, else 4-wide ones (two CTAs per SM: one gathers while the other computes)
         const size_t smem8 = (size_t)k3_tile_rows(nx) * 8 * sizeof(cplx) + (size_t)10 * ((nx + 15) / 16) * 8 * sizeof(double)
-                             + (size_t)k3_coef_slots(nx, 16) * (sizeof(double2) + (MODE == 1 ? sizeof(double) : 0)) + 128;
+                             + (size_t)k3_coef_slots(nx, 16) * sizeof(double2) + 128;
         if (2 * (smem8 + 1024) > 228 * 1024) kw = 4;
         if (getenv("AFID_K3_KW")) kw = atoi(getenv("AFID_K3_KW")) == 4 ? 4 : 8;
-        if (kw == 8) c.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 8, MODE> : (const void*)k_solve_x<16, false, true, 8, MODE>;
-        else c.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 4, MODE> : (const void*)k_solve_x<16, false, true, 4, MODE>;
+        if (kw == 8) c.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 8 > : (const void*)k_solve_x<16, false, true, 8 >;
+        else c.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 4 > : (const void*)k_solve_x<16, false, true, 4 >;
     }
-    else { M = 32; c.fn = (nx % 32 == 0) ? (const void*)k_solve_x<32, true, false, 8, MODE> : (const void*)k_solve_x<32, false, false, 8, MODE>; }
+    else { M = 32; c.fn = (nx % 32 == 0) ? (const void*)k_solve_x<32, true, false, 8 > : (const void*)k_solve_x<32, false, false, 8 >; }
     const int pch = (nx + M - 1) / M;
     c.threads = kw * pch;
     c.smem = (size_t)k3_tile_rows(nx) * kw * sizeof(cplx) + (size_t)10 * pch * kw * sizeof(double)
-             + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * (sizeof(double2) + (MODE == 1 ? sizeof(double) : 0)) : 0) + 128;
+             + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * sizeof(double2) : 0) + 128;
     c.ctas_per_sm = 4;
     c.nl = 0;
     *kw_out = kw;
@@ -282,7 +282,7 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
 
     // ---- K3 configuration
-    pl->k3 = select_k3<0>(nx, &pl->k3_kw);
+    pl->k3 = select_k3(nx, &pl->k3_kw);
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -519,40 +519,107 @@ int afid_plan_set_accumulate(afid_plan* pl, int on)
 // ---- batched real tridiagonal solves in x on a field (implicit wall-normal step) ----------
 struct afid_xsolve {
     afid_plan* pl;
-    DevParams dp;      // the plan's parameters with ca, cc, rowlam pointing at this object's tables
+    DevParams dp;
     LaunchCfg k;
-    int kw;
-    double* tables;    // device: a[nx], c[nx], lam[nx]
+    XsTables xt;       // device tables of the row-only quantities (k_xsolve_field)
+    void* tables;      // one device allocation holding them
 };
 
-afid_xsolve* afid_xsolve_create(afid_plan* pl, const double* a, const double* c, const double* lam)
+afid_xsolve* afid_xsolve_create(afid_plan* pl, const double* a_in, const double* c_in, const double* lam)
 {
     g_err.clear();
     g_err_code = 0;
-    if (!pl || !a || !c || !lam) { fail(AFID_ERR_NULL, "plan, a, c or lam is NULL"); return nullptr; }
+    if (!pl || !a_in || !c_in || !lam) { fail(AFID_ERR_NULL, "plan, a, c or lam is NULL"); return nullptr; }
     const int nx = pl->nx;
     for (int i = 0; i < nx; ++i)
-        if (!(a[i] >= 0.0) || !(c[i] >= 0.0) || !(lam[i] > 0.0) || !std::isfinite(a[i]) || !std::isfinite(c[i]) || !std::isfinite(lam[i])) {
+        if (!(a_in[i] >= 0.0) || !(c_in[i] >= 0.0) || !(lam[i] > 0.0) || !std::isfinite(a_in[i]) || !std::isfinite(c_in[i]) || !std::isfinite(lam[i])) {
             fail(AFID_ERR_GRID, "afid_xsolve_create needs finite a_i >= 0, c_i >= 0, lam_i > 0 (an M-matrix)");
             return nullptr;
         }
     afid_xsolve* h = new (std::nothrow) afid_xsolve();
     if (!h) { fail(AFID_ERR_NOMEM, "host allocation failed"); return nullptr; }
     h->pl = pl;
-    h->k = select_k3<1>(nx, &h->kw);
-    if (set_smem_attr(h->k) != AFID_OK) { delete h; return nullptr; }
-    if (cudaMalloc((void**)&h->tables, 3 * (size_t)nx * sizeof(double)) != cudaSuccess) {
-        cudaGetLastError(); delete h; fail(AFID_ERR_NOMEM, "cudaMalloc(xsolve tables) failed"); return nullptr;
-    }
-    std::vector<double> t(3 * (size_t)nx);
-    for (int i = 0; i < nx; ++i) { t[i] = (i == 0) ? 0.0 : a[i]; t[nx + i] = (i == nx - 1) ? 0.0 : c[i]; t[2 * nx + i] = lam[i]; }
-    if (cudaMemcpy(h->tables, t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) {
-        cudaFree(h->tables); delete h; fail(AFID_ERR_CUDA, "cudaMemcpy(xsolve tables) failed"); return nullptr;
-    }
     h->dp = pl->dp;
-    h->dp.ca = h->tables;
-    h->dp.cc = h->tables + nx;
-    h->dp.rowlam = h->tables + 2 * nx;
+    const int M = (nx < 64) ? 4 : (nx <= 1024 ? 16 : 32);
+    const int KW = (nx <= 1024) ? 8 : 4;   // 128-byte rows wherever the tile fits shared memory
+    const int PCH = (nx + M - 1) / M;
+    if (KW == 4) h->k.fn = (M == 4) ? (const void*)k_xsolve_field<4, 4> : (M == 16 ? (const void*)k_xsolve_field<16, 4> : (const void*)k_xsolve_field<32, 4>);
+    else h->k.fn = (M == 4) ? (const void*)k_xsolve_field<4, 8> : (const void*)k_xsolve_field<16, 8>;
+    h->k.threads = PCH * KW;
+    h->k.smem = (size_t)k3_tile_rows(nx) * KW * sizeof(cplx) + (size_t)2 * PCH * KW * sizeof(cplx) + 128;
+    h->k.ctas_per_sm = 3;
+    h->k.nl = KW;   // (complex lanes per tile)
+    if (set_smem_attr(h->k) != AFID_OK) { delete h; return nullptr; }
+
+    // ---- the row-only quantities of the partitioned solve, in long double (same algebra as k_solve_x)
+    typedef long double ld;
+    std::vector<ld> a(nx), c(nx);
+    for (int i = 0; i < nx; ++i) { a[i] = (i == 0) ? 0.0L : (ld)a_in[i]; c[i] = (i == nx - 1) ? 0.0L : (ld)c_in[i]; }
+    std::vector<double> UP(2 * (size_t)nx, 0.0), DN(2 * (size_t)nx, 0.0), GH(2 * (size_t)nx, 0.0), CH(2 * (size_t)PCH, 0.0), RE(PCH, 0.0);
+    std::vector<ld> A(PCH, 0.0L), C(PCH, 0.0L), L(PCH, 0.0L), hup(PCH, 1.0L), tup(PCH, 0.0L);
+    for (int q = 0; q < PCH; ++q) {
+        const int i0 = q * M, i1 = std::min(i0 + M, nx) - 1;
+        ld hh = 1.0L, tt = 0.0L;
+        for (int i = i1 - 1; i >= i0; --i) {                    // upward
+            const ld nh = c[i] * hh, nt = (ld)lam[i] + c[i] * tt, rr = 1.0L / (a[i] + (nh + nt));
+            hh = nh * rr; tt = nt * rr;
+            UP[2 * i] = (double)(c[i] * rr); UP[2 * i + 1] = (double)rr;
+        }
+        hup[q] = hh; tup[q] = tt;
+        hh = 1.0L; tt = 0.0L;
+        for (int i = i0; i < i1; ++i) {                         // downward
+            const ld nh = a[i] * hh, nt = (ld)lam[i] + a[i] * tt, rr = 1.0L / (c[i] + (nh + nt));
+            hh = nh * rr; tt = nt * rr;
+            DN[2 * i] = (double)(a[i] * rr); DN[2 * i + 1] = (double)rr;
+            GH[2 * i] = (double)(c[i] * rr); GH[2 * i + 1] = (double)hh;
+        }
+        const ld ab = a[i1], cb = (q > 0) ? c[i0 - 1] : 0.0L;
+        CH[2 * q] = (double)ab; CH[2 * q + 1] = (double)cb;
+        A[q] = ab * hh;
+        L[q] = (ld)lam[i1] + ab * tt;
+    }
+    for (int q = 0; q + 1 < PCH; ++q) {                          // the next chunk's upward relation enters row q
+        const ld cb = c[(q + 1) * M - 1];
+        C[q] = cb * hup[q + 1];
+        L[q] += cb * tup[q + 1];
+    }
+    int nlev = 0;
+    for (int d = 1; d < PCH; d <<= 1) ++nlev;
+    std::vector<double> PC(2 * (size_t)std::max(nlev, 1) * PCH, 0.0);
+    {
+        int lev = 0;
+        for (int d = 1; d < PCH; d <<= 1, ++lev) {
+            std::vector<ld> A2(PCH, 0.0L), C2(PCH, 0.0L), L2(L);
+            for (int q = 0; q < PCH; ++q) {
+                ld al = 0.0L, ga = 0.0L;
+                if (q - d >= 0) { const int m = q - d; al = A[q] / (A[m] + C[m] + L[m]); A2[q] = al * A[m]; L2[q] += al * L[m]; }
+                if (q + d < PCH) { const int m = q + d; ga = C[q] / (A[m] + C[m] + L[m]); C2[q] = ga * C[m]; L2[q] += ga * L[m]; }
+                PC[2 * ((size_t)lev * PCH + q)] = (double)al;
+                PC[2 * ((size_t)lev * PCH + q) + 1] = (double)ga;
+            }
+            A = A2; C = C2; L = L2;
+        }
+    }
+    for (int q = 0; q < PCH; ++q) RE[q] = (double)(1.0L / (A[q] + C[q] + L[q]));
+
+    struct Item { const void* src; size_t bytes; size_t off; };
+    std::vector<Item> items = {{UP.data(), UP.size() * 8, 0}, {DN.data(), DN.size() * 8, 0}, {GH.data(), GH.size() * 8, 0},
+                               {CH.data(), CH.size() * 8, 0}, {RE.data(), RE.size() * 8, 0}, {PC.data(), PC.size() * 8, 0}};
+    size_t off = 0;
+    for (auto& it : items) { it.off = off; off += (it.bytes + 255) / 256 * 256; }
+    if (cudaMalloc(&h->tables, off) != cudaSuccess) { cudaGetLastError(); delete h; fail(AFID_ERR_NOMEM, "cudaMalloc(xsolve tables) failed"); return nullptr; }
+    for (auto& it : items)
+        if (cudaMemcpy((char*)h->tables + it.off, it.src, it.bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaFree(h->tables); delete h; fail(AFID_ERR_CUDA, "cudaMemcpy(xsolve tables) failed"); return nullptr;
+        }
+    char* tb = (char*)h->tables;
+    h->xt.UP = (const double2*)(tb + items[0].off);
+    h->xt.DN = (const double2*)(tb + items[1].off);
+    h->xt.GH = (const double2*)(tb + items[2].off);
+    h->xt.CH = (const double2*)(tb + items[3].off);
+    h->xt.RE = (const double*)(tb + items[4].off);
+    h->xt.PC = (const double2*)(tb + items[5].off);
+    h->xt.nlev = nlev;
     return h;
 }
 
@@ -563,12 +630,12 @@ int afid_xsolve_apply(afid_xsolve* h, double* f, void* stream)
     if ((rc = check_ptr(f, "f"))) return rc;
     const afid_plan* pl = h->pl;
     alignas(64) CUtensorMap map;
-    if (!make_map3(&map, f, (uint64_t)pl->nz, (uint64_t)pl->ny, (uint64_t)pl->nx, 2 * (uint32_t)h->kw, 1, (uint32_t)k3_box_rows(pl->nx),
+    if (!make_map3(&map, f, (uint64_t)pl->nz, (uint64_t)pl->ny, (uint64_t)pl->nx, 2 * (uint32_t)h->k.nl, 1, (uint32_t)k3_box_rows(pl->nx),
                    CU_TENSOR_MAP_SWIZZLE_NONE))
         return fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed");
     cplx* fc = reinterpret_cast<cplx*>(f);
-    void* args[] = {&h->dp, (void*)&map, (void*)&fc};
-    return launch(h->k, (unsigned)(pl->ny * ((pl->nz / 2) / h->kw)), (cudaStream_t)stream, args, "k_solve_x(field)");
+    void* args[] = {&h->dp, &h->xt, (void*)&map, (void*)&fc};
+    return launch(h->k, (unsigned)(pl->ny * ((pl->nz / 2) / h->k.nl)), (cudaStream_t)stream, args, "k_xsolve_field");
 }
 
 int afid_xsolve_destroy(afid_xsolve* h)
