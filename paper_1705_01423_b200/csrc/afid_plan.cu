@@ -263,6 +263,16 @@ static int set_smem_attr(const LaunchCfg& c)
     return AFID_OK;
 }
 
+// free whatever a partially built plan holds (the struct is zero-initialised; cudaFree(nullptr) is a no-op)
+static void discard_plan(afid_plan* pl)
+{
+    cudaFree(pl->ws[0]);
+    cudaFree(pl->ws[1]);
+    cudaFree(pl->tables);
+    cudaFree(pl->sync56);
+    delete pl;
+}
+
 afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly, double Lz)
 {
     g_err.clear();
@@ -337,33 +347,32 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     size_t off = 0;
     for (auto& it : items) { it.off = off; off += (it.bytes + 255) / 256 * 256; }
     pl->tables_bytes = off;
-    if (cudaMalloc(&pl->tables, off) != cudaSuccess) { cudaGetLastError(); delete pl; fail(AFID_ERR_NOMEM, "cudaMalloc(tables) failed"); return nullptr; }
+    if (cudaMalloc(&pl->tables, off) != cudaSuccess) { cudaGetLastError(); discard_plan(pl); fail(AFID_ERR_NOMEM, "cudaMalloc(tables) failed"); return nullptr; }
     for (auto& it : items)
         if (cudaMemcpy((char*)pl->tables + it.off, it.src, it.bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
-            cudaFree(pl->tables); delete pl; fail(AFID_ERR_CUDA, "cudaMemcpy(tables) failed"); return nullptr;
+            discard_plan(pl); fail(AFID_ERR_CUDA, "cudaMemcpy(tables) failed"); return nullptr;
         }
     pl->fuse56 = getenv("AFID_FUSE56") && atoi(getenv("AFID_FUSE56")) == 1; // off by default: slower than K5 + K6
     {
         const size_t nflag = 1 + (size_t)nx * (ny / 8);
         if (cudaMalloc((void**)&pl->sync56, nflag * sizeof(unsigned)) != cudaSuccess || cudaMemset(pl->sync56, 0, nflag * sizeof(unsigned)) != cudaSuccess) {
-            cudaGetLastError(); cudaFree(pl->tables); delete pl; fail(AFID_ERR_NOMEM, "cudaMalloc(flags) failed"); return nullptr;
+            cudaGetLastError(); discard_plan(pl); fail(AFID_ERR_NOMEM, "cudaMalloc(flags) failed"); return nullptr;
         }
     }
     pl->ws_bytes = (size_t)nx * pl->nzh * ny * sizeof(cplx);
     for (int b = 0; b < 2; ++b)
         if (cudaMalloc((void**)&pl->ws[b], pl->ws_bytes) != cudaSuccess) {
             cudaGetLastError();
-            if (b == 1) cudaFree(pl->ws[0]);
-            cudaFree(pl->tables); delete pl; fail(AFID_ERR_NOMEM, "cudaMalloc(work arrays) failed"); return nullptr;
+            discard_plan(pl); fail(AFID_ERR_NOMEM, "cudaMalloc(work arrays) failed"); return nullptr;
         }
     if (!make_map3(&pl->mapC, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)nx, (uint64_t)pl->nzh, 2 * (uint32_t)pl->k3_kw, (uint32_t)k3_box_rows(nx), 1,
                    CU_TENSOR_MAP_SWIZZLE_NONE)) {
-        cudaFree(pl->ws[0]); cudaFree(pl->ws[1]); cudaFree(pl->tables); delete pl;
+        discard_plan(pl);
         fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed"); return nullptr;
     }
     if (!make_map3(&pl->mapD, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)pl->nzh, (uint64_t)nx, 16, (uint32_t)k5_box_rows(nh), 1,
                    CU_TENSOR_MAP_SWIZZLE_128B)) {
-        cudaFree(pl->ws[0]); cudaFree(pl->ws[1]); cudaFree(pl->tables); delete pl;
+        discard_plan(pl);
         fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed"); return nullptr;
     }
     char* tb = (char*)pl->tables;
