@@ -86,6 +86,10 @@ SHAPES = [
     dict(nx=2, ny=1280, nz=640, grid="uniform"),
     dict(nx=2, ny=2560, nz=80, grid="tanh", s=3.0),
     dict(nx=5, ny=320, nz=80, grid="tanh", s=3.0),
+    # the largest instantiations: nz/2 = 1024, ny = 3072, nx = afid_max_nx()
+    dict(nx=3, ny=8, nz=2048, grid="uniform"),
+    dict(nx=2, ny=3072, nz=16, grid="uniform"),
+    dict(nx=1536, ny=8, nz=16, grid="tanh", s=3.0),
 ]
 
 
