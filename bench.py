@@ -227,6 +227,29 @@ def run_gpu(args):
             e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
 
     peak, peak_src = measured_peaks()
+    # SURVEY.md 8(f) rows, timed outside the step: afid_max_cfl (24 B/pt) and afid_xsolve_apply (16 B/pt)
+    extras = {}
+    try:
+        def timed(fn, reps=5):
+            for _ in range(2):
+                fn()
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0.record(stream)
+            for _ in range(reps):
+                fn()
+            t1.record(stream)
+            torch.cuda.synchronize()
+            return t0.elapsed_time(t1) / reps
+        out = torch.empty(1, dtype=torch.float64, device=dev)
+        ms_cfl = timed(lambda: plan.max_cfl(u, v, w, out))
+        dxs = np.diff(xc)
+        xs = plan.xsolve(np.r_[0.0, 1.0 / dxs[1:] ** 2], np.r_[1.0 / dxs[:-1] ** 2, 0.0], np.full(nx, 1.0e3))
+        ms_xs = timed(lambda: xs.apply(p))
+        xs.destroy()
+        extras = {"afid_max_cfl": {"ms": ms_cfl, "alg_GBps": 24.0 * N / (ms_cfl * 1e-3) / 1e9, "frac_of_peak": 24.0 * N / (ms_cfl * 1e-3) / 1e9 / peak},
+                  "afid_xsolve_apply": {"ms": ms_xs, "alg_GBps": 16.0 * N / (ms_xs * 1e-3) / 1e9, "frac_of_peak": 16.0 * N / (ms_xs * 1e-3) / 1e9 / peak}}
+    except Exception as ex:
+        extras = {"error": str(ex)[:200]}
     dom = max(kt, key=kt.get)
     ach = ALG_BYTES_PER_POINT[dom] * N / (kt[dom] * 1e-3) / 1e9
     traffic = ncu_traffic(dom) if args.workload == "C4" else None
@@ -243,7 +266,7 @@ def run_gpu(args):
               "l2": "working set (>= 77 GB) far larger than the 126 MB L2; no flush needed",
               "device_bytes": plan.workspace_bytes + (4 * N + ny * nz) * 8}
     line = make_line(config, world, args.steps, args.warmup, ms_total, pts, clocks=clocks, e2e=e2e,
-                     gpu_launches=plan.num_launches * args.steps, roofline=roofline, kernels=kernels,
+                     gpu_launches=plan.num_launches * args.steps, roofline=roofline, kernels=kernels, extras=extras,
                      path_roofline={"alg_bytes_per_point": PATH_ALG_BYTES_PER_POINT, "achieved_GBps": path_gbs,
                                     "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS, "frac_of_measured": path_gbs / peak})
     if rank == 0 and not args.no_cpu_baseline and world == 1:
