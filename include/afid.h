@@ -72,6 +72,8 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
  * (steps 2,4,6,8,10,12, the pencil transposes, are folded into the kernels' tile loads).
  * Returns AFID_OK or a negative code.  Validation is synchronous; the kernels are only
  * enqueued, so execution errors surface at the caller's next synchronisation.
+ * The call only enqueues kernels (and, with timing enabled, event records) on `stream`, so it may be captured
+ * in a CUDA graph and replayed.
  * NaN/Inf in the inputs propagate.  The compatibility condition (zero net wall flux) is
  * not checked; it holds identically when u vanishes on both wall planes.
  */

@@ -174,6 +174,35 @@ def test_xsolve_parity(shape):
     plan.destroy()
 
 
+def test_cuda_graph_capture_replays_bit_identically():
+    """afid_project only enqueues kernels on the given stream, so it can be captured in a CUDA graph
+    (C1 is launch-latency bound: six launches; a replay takes about half the eager time)."""
+    cfg = synth.config("C1")
+    xc = synth.grid_faces(cfg)
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    u, v, w = synth.velocity(cfg, xc)
+    u0, v0, w0 = u.cuda(), v.cuda(), w.cuda()
+    ud, vd, wd = u0.clone(), v0.clone(), w0.clone()
+    p = torch.empty_like(vd)
+    plan = afid.Plan(nx, ny, nz, xc, cfg["Ly"], cfg["Lz"])
+    plan.project(ud, vd, wd, p)
+    torch.cuda.synchronize()
+    eager = (ud.clone(), vd.clone(), wd.clone(), p.clone())
+    s = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    ud.copy_(u0); vd.copy_(v0); wd.copy_(w0)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            plan.project(ud, vd, wd, p, stream=torch.cuda.current_stream())
+    for _ in range(2):
+        ud.copy_(u0); vd.copy_(v0); wd.copy_(w0); p.fill_(float("nan"))
+        g.replay()
+        torch.cuda.synchronize()
+        assert all(torch.equal(a, b) for a, b in zip(eager, (ud, vd, wd, p)))
+    plan.destroy()
+
+
 def test_accumulate_mode_parity():
     """afid_plan_set_accumulate(1): p_out = p_in + phi (P:L91, P:L116 delta form); the velocities as before."""
     cfg = synth.config("C1", nx=40, ny=64, nz=128, grid="tanh", s=3.0)
