@@ -369,6 +369,8 @@ def _full_size_checks(name, sample_planes):
     us = torch.empty_like(u)
     mf.solenoidal_into(cfg, xc, psi, chi, us, phi, psi)   # v_sol -> phi's storage, w_sol -> psi's storage
     e_u, e_v, e_w = mf.rel_l2(u, us), mf.rel_l2(v, phi), mf.rel_l2(w, psi)
+    print(f"{name}: rel L2 vs the manufactured answer p {e_p:.2e} u {e_u:.2e} v {e_v:.2e} w {e_w:.2e}; "
+          f"max|div_out|/max|div_in| = {div_out / div_in:.2e}")
     assert max(e_p, e_u, e_v, e_w) <= TOL, dict(p=e_p, u=e_u, v=e_v, w=e_w)
 
 
