@@ -680,12 +680,14 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const dou
 // Parallel-in-x algorithm, every quantity a sum/product of non-negative numbers (no
 // cancellation at small lam):
 //   chunk q = rows [qM, qM+M); its last row is an INTERFACE unknown E_q, the others are interior.
-//   interior row elimination toward a boundary carries  x_i = y_i + g_i x_next + h_i E_far
-//   with g + h + t = 1 and   nh = a h', nt = lam + a t', pi = c + nh + nt,
-//                            h = nh/pi, t = nt/pi, g = c/pi, y = (f + a y')/pi      (downward; upward: a<->c)
+//   1. downward elimination of the interior (one reciprocal per row):  x_i = y_i + g_i x_{i+1} + h_i E_{q-1}
+//        nh = a h', nt = lam + a t', pi = c + nh + nt, h = nh/pi, t = nt/pi, g = c/pi, y = (f + a y')/pi   (g + h + t = 1)
+//   2. in the same sweep, by prefix products Pg = g_0 ... g_{r-1}: the chunk's FIRST interior row in terms of
+//      both interfaces,  x_{i0} = Y + Gq E_q + Hq E_{q-1},   Y = sum Pg y_r, Hq = sum Pg h_r, Gq = prod g,
+//      Tq = 1 - Gq - Hq = sum Pg t_r  (a sum of non-negatives)
 //   -> reduced system in E of the same form: -A_q E_{q-1} + (A_q + C_q + L_q) E_q - C_q E_{q+1} = F_q
-//      A_q = a h, C_q = c h^, L_q = lam + a t + c t^, F_q = f + a y + c y^
-//   -> solved by cancellation-free parallel cyclic reduction across the P threads of a system
+//        A_q = a h, L_q = lam + a t + c Tq^, F_q = f + a y + c Y^, C_q = c Gq^   (^ = chunk q+1's first-row relation)
+//   -> solved by cancellation-free parallel cyclic reduction across the chunks of a system
 //      (L' = L + alpha L_- + gamma L_+ stays a sum of non-negatives)
 //   -> interior rows by back substitution x_i = y_i + g_i x_{i+1} + h_i E_{q-1}.
 // Mode (0,0) (lam = 0, singular; R7): last row pinned to 0, then the dx-weighted
@@ -713,10 +715,8 @@ __device__ __forceinline__ double fast_rcp(double x)
 }
 
 
-// EXACT: nx is a multiple of M (every chunk is full: no per-row bounds checks).
-// COEF_SMEM: the coefficients {a_i, c_i} are staged in shared memory (one conflict-free LDS.128 per
-// row instead of two global loads); not for the largest nx, where the tile fills shared memory.
-template <int M> constexpr int k3_threads() { return M == 4 ? 128 : (M == 16 ? 512 : 384); }
+// EXACT: nx is a multiple of M (every chunk is full: no per-row bounds checks).  The coefficients {a_i, c_i}
+// are staged in shared memory (one conflict-free LDS.128 per row, one pad slot per chunk).
 __host__ __device__ constexpr int k3_coef_slots(int nx, int M) { return nx + nx / M + 1; }
 
 // rows per TMA box of the K3 tile gather (box = 8 ky x 1 kz x k3_box_rows(nx) planes), and the rows the
@@ -727,8 +727,9 @@ __host__ __device__ constexpr int k3_tile_rows(int nx) { return k3_num_boxes(nx)
 
 // KW = systems (consecutive ky) per CTA: 8 (128-byte rows), or 4 (64-byte rows; half the shared memory, so that
 // two CTAs share an SM and one gathers while the other computes -- used when the 8-wide tile allows only one).
-template <int M, bool EXACT, bool COEF_SMEM, int KW>
-__global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams P, const __grid_constant__ CUtensorMap mapC, cplx* __restrict__ T)
+// TB = thread bound of the instantiation (KW times the largest number of chunks it is launched with).
+template <int M, bool EXACT, int KW, int TB>
+__global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_constant__ CUtensorMap mapC, cplx* __restrict__ T)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
@@ -754,17 +755,10 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         mbar_expect_tx(&bar, (uint32_t)(nb * br * KW * sizeof(cplx)));
         for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * KW, &mapC, ky0 * 2, b * br, kz, &bar, pol);
     }
-    if (COEF_SMEM) {
-        for (int i = threadIdx.x; i < nx; i += blockDim.x) coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
-        __syncthreads();
-    }
+    for (int i = threadIdx.x; i < nx; i += blockDim.x) coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
+    __syncthreads();
     mbar_wait(&bar, 0);
-    // coefficients {a_i, c_i} of row i; `cq` = slot of the chunk's first row (slot(i) = i + i/M = cq + (i - qM))
-    const double2* cq = coef + (size_t)(threadIdx.x / KW) * (M + 1);
-    auto ld_ac = [&](int i) -> double2 {
-        if (COEF_SMEM) return coef[i + i / M];
-        return make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
-    };
+    auto ld_ac = [&](int i) -> double2 { return coef[i + i / M]; };   // {a_i, c_i}: one conflict-free LDS.128
     const double lam = __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]);
     const bool cta_singular = (blockIdx.x == 0);
     const int i0 = q * M;
@@ -780,89 +774,17 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
     double* nFr = nA + 3 * NS;
     double* nFi = nA + 4 * NS;
 
-    double G[M - 1 > 0 ? M - 1 : 1], H[M - 1 > 0 ? M - 1 : 1];
+    constexpr int MI = (M - 1 > 0) ? M - 1 : 1;
+    double G[MI], H[MI];
     double rA, rC, rL, rFr, rFi;
-    // Interior elimination of the chunk in both directions.  Upward (read only): relation of the first
-    // interior row to the interface above.  Downward (in place: tile <- y), keeping g, h in registers.
-    // The two recurrences are independent dependency chains; for full chunks they are interleaved row
-    // by row (twice the instruction-level parallelism); the downward sweep overwrites f with y, so the
-    // f of the first (M-1)/2 rows is kept in registers for the upward sweep, which reaches them last.
-    constexpr bool INTERLEAVE = EXACT && (M <= 16);
-    if constexpr (INTERLEAVE) {
-        constexpr int NF = (M - 1) / 2 > 0 ? (M - 1) / 2 : 1;
-        cplx F[NF];
-        double hu = 1.0, tu = 0.0, yur = 0.0, yui = 0.0;
-        double hd = 1.0, td = 0.0, ydr = 0.0, ydi = 0.0;
-#pragma unroll
-        for (int k = 0; k < M - 1; ++k) {
-            {   // upward, row ru = M-2-k (rows 0..k-1 already hold y: take f from the register copy)
-                const int ru = M - 2 - k;
-                const double2 ac = ld_ac(i0 + ru);
-                const double a = ac.x, c = ac.y;
-                const cplx f = (ru >= k) ? tile[(i0 + ru) * KW + s] : F[ru < NF ? ru : 0];
-                const double nh = c * hu, nt = fma(c, tu, lam);
-                const double rr = fast_rcp(a + (nh + nt));
-                hu = nh * rr;
-                tu = nt * rr;
-                yur = fma(c, yur, f.x) * rr;
-                yui = fma(c, yui, f.y) * rr;
-            }
-            {   // downward, row k
-                const double2 ac = ld_ac(i0 + k);
-                const double a = ac.x, c = ac.y;
-                const cplx f = tile[(i0 + k) * KW + s];
-                if (k < NF && k < (M - 1) / 2) F[k] = f;
-                const double nh = a * hd, nt = fma(a, td, lam);
-                const double rr = fast_rcp(c + (nh + nt));
-                hd = nh * rr;
-                td = nt * rr;
-                ydr = fma(a, ydr, f.x) * rr;
-                ydi = fma(a, ydi, f.y) * rr;
-                tile[(i0 + k) * KW + s] = mk(ydr, ydi);
-                G[k] = c * rr;
-                H[k] = hd;
-            }
-        }
-        if (q > 0) { // contribution to the interface row above (reduced row q-1); staged in the "next" buffer
-            const double cb = COEF_SMEM ? coef[(i0 - 1) + (i0 - 1) / M].y : __ldg(&P.cc[i0 - 1]); // (previous chunk's last row)
-            nC[slot - KW] = cb * hu;
-            nL[slot - KW] = cb * tu;
-            nFr[slot - KW] = cb * yur;
-            nFi[slot - KW] = cb * yui;
-        }
-        const double ab = ld_ac(i1).x;
-        const cplx f = tile[i1 * KW + s];
-        rA = ab * hd;
-        rL = fma(ab, td, lam);
-        rFr = fma(ab, ydr, f.x);
-        rFi = fma(ab, ydi, f.y);
-    } else {
-        {
-            double h = 1.0, t = 0.0, yr = 0.0, yi = 0.0;
-#pragma unroll
-            for (int r = M - 2; r >= 0; --r) {
-                const int i = i0 + r;
-                if (EXACT || i < i1) {
-                    const double2 ac = ld_ac(i);
-                    const double a = ac.x, c = ac.y;
-                    const double nh = c * h, nt = fma(c, t, lam);
-                    const double rr = fast_rcp(a + (nh + nt));
-                    const cplx f = tile[i * KW + s];
-                    h = nh * rr;
-                    t = nt * rr;
-                    yr = fma(c, yr, f.x) * rr;
-                    yi = fma(c, yi, f.y) * rr;
-                }
-            }
-            if (q > 0) {
-                const double cb = COEF_SMEM ? coef[(i0 - 1) + (i0 - 1) / M].y : __ldg(&P.cc[i0 - 1]); // (previous chunk's last row)
-                nC[slot - KW] = cb * h;
-                nL[slot - KW] = cb * t;
-                nFr[slot - KW] = cb * yr;
-                nFi[slot - KW] = cb * yi;
-            }
-        }
+    {   // ONE elimination sweep over the chunk interior, in place (tile <- y), one reciprocal per row:
+        //   x_i = y_i + g_i x_{i+1} + h_i E_{q-1},   g + h + t = 1.
+        // Along the way the first interior row is expressed in the two interfaces by prefix products of g
+        // (Pg = g_0 ... g_{r-1}):   x_{i0} = Y + Gq E_q + Hq E_{q-1},
+        //   Y = sum Pg y_r,  Hq = sum Pg h_r,  Gq = g_0 ... g_last,  Tq = 1 - Gq - Hq = sum Pg t_r  (no cancellation)
+        // -- what the interface above needs for its reduced row, without a second (upward) elimination.
         double h = 1.0, t = 0.0, yr = 0.0, yi = 0.0;
+        double Pg = 1.0, Yr = 0.0, Yi = 0.0, Hq = 0.0, Tq = 0.0;
 #pragma unroll
         for (int r = 0; r < M - 1; ++r) {
             const int i = i0 + r;
@@ -877,9 +799,22 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
                 yr = fma(a, yr, f.x) * rr;
                 yi = fma(a, yi, f.y) * rr;
                 tile[i * KW + s] = mk(yr, yi);
-                G[r] = c * rr;
+                const double g = c * rr;
+                G[r] = g;
                 H[r] = h;
+                Yr = fma(Pg, yr, Yr);
+                Yi = fma(Pg, yi, Yi);
+                Hq = fma(Pg, h, Hq);
+                Tq = fma(Pg, t, Tq);
+                Pg *= g;
             }
+        }
+        if (q > 0) { // contribution to the interface row above (reduced row q-1); staged in the "next" buffer
+            const double cb = coef[(i0 - 1) + (i0 - 1) / M].y;
+            nC[slot - KW] = cb * Pg;
+            nL[slot - KW] = cb * Tq;
+            nFr[slot - KW] = cb * Yr;
+            nFi[slot - KW] = cb * Yi;
         }
         const double ab = ld_ac(i1).x;
         const cplx f = tile[i1 * KW + s];
@@ -942,12 +877,11 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
         const double elr = (q > 0) ? bFr[slot - KW] : 0.0, eli = (q > 0) ? bFi[slot - KW] : 0.0;
         double xr = er, xi = ei;
         // T[kz][kyt][i][8]: the tile is contiguous in global memory.  All CTAs but the one holding the
-        // mean mode store x straight from the back substitution (128-byte segments per row; the stores
+        // mean mode store x straight from the back substitution (64/128-byte segments per row; the stores
         // drain while the next CTA of this SM already loads its tile).
         cplx* dst = T + ((size_t)kz * nkt + ky0 / 8) * (size_t)nx * 8 + (ky0 % 8);
-        constexpr int rstride = 8;
         if (!cta_singular) {
-            dst[i1 * rstride + s] = mk(xr, xi);
+            dst[i1 * 8 + s] = mk(xr, xi);
 #pragma unroll
             for (int r = M - 2; r >= 0; --r) {
                 const int i = i0 + r;
@@ -955,7 +889,7 @@ __global__ void __launch_bounds__(k3_threads<M>() * KW / 8) k_solve_x(DevParams 
                     const cplx y = tile[i * KW + s];
                     xr = fma(G[r], xr, fma(H[r], elr, y.x));
                     xi = fma(G[r], xi, fma(H[r], eli, y.y));
-                    dst[i * rstride + s] = mk(xr, xi);
+                    dst[i * 8 + s] = mk(xr, xi);
                 }
             }
             return;

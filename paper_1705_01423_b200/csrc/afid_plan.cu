@@ -155,22 +155,23 @@ LaunchCfg select_k3(int nx, int* kw_out)
 {
     LaunchCfg c{};
     int M, kw = 8;
-    if (nx < 64) { M = 4; c.fn = (nx % 4 == 0) ? (const void*)k_solve_x<4, true, true, 8 > : (const void*)k_solve_x<4, false, true, 8 >; }
-    else if (nx <= 1024) {
+    if (nx < 64) { M = 4; c.fn = (nx % 4 == 0) ? (const void*)k_solve_x<4, true, 8, 128> : (const void*)k_solve_x<4, false, 8, 128>; }
+    else {
         M = 16;
         // 8-wide tiles if two of them fit an SM, else 4-wide ones (two CTAs per SM: one gathers while the other computes)
         const size_t smem8 = (size_t)k3_tile_rows(nx) * 8 * sizeof(cplx) + (size_t)10 * ((nx + 15) / 16) * 8 * sizeof(double)
                              + (size_t)k3_coef_slots(nx, 16) * sizeof(double2) + 128;
         if (2 * (smem8 + 1024) > 228 * 1024) kw = 4;
-        if (getenv("AFID_K3_KW")) kw = atoi(getenv("AFID_K3_KW")) == 4 ? 4 : 8;
-        if (kw == 8) c.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 8 > : (const void*)k_solve_x<16, false, true, 8 >;
-        else c.fn = (nx % 16 == 0) ? (const void*)k_solve_x<16, true, true, 4 > : (const void*)k_solve_x<16, false, true, 4 >;
+        if (getenv("AFID_K3_KW") && nx <= 1024) kw = atoi(getenv("AFID_K3_KW")) == 4 ? 4 : 8;
+        const bool ex = (nx % 16 == 0);
+        if (kw == 8) c.fn = ex ? (const void*)k_solve_x<16, true, 8, 512> : (const void*)k_solve_x<16, false, 8, 512>;
+        else if (nx <= 1024) c.fn = ex ? (const void*)k_solve_x<16, true, 4, 256> : (const void*)k_solve_x<16, false, 4, 256>;
+        else c.fn = ex ? (const void*)k_solve_x<16, true, 4, 384> : (const void*)k_solve_x<16, false, 4, 384>;
     }
-    else { M = 32; c.fn = (nx % 32 == 0) ? (const void*)k_solve_x<32, true, false, 8 > : (const void*)k_solve_x<32, false, false, 8 >; }
     const int pch = (nx + M - 1) / M;
     c.threads = kw * pch;
     c.smem = (size_t)k3_tile_rows(nx) * kw * sizeof(cplx) + (size_t)10 * pch * kw * sizeof(double)
-             + (M <= 16 ? (size_t)k3_coef_slots(nx, M) * sizeof(double2) : 0) + 128;
+             + (size_t)k3_coef_slots(nx, M) * sizeof(double2) + 128;
     c.ctas_per_sm = 4;
     c.nl = 0;
     *kw_out = kw;
