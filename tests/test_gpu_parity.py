@@ -203,6 +203,24 @@ def test_cuda_graph_capture_replays_bit_identically():
     plan.destroy()
 
 
+def test_bitwise_deterministic():
+    """No atomics and no data-dependent scheduling on the default path: the same input gives the same bits."""
+    cfg = synth.config("C2", nx=128, ny=96, nz=192)
+    xc = synth.grid_faces(cfg)
+    u, v, w = synth.velocity(cfg, xc)
+    plan = afid.Plan(cfg["nx"], cfg["ny"], cfg["nz"], xc, cfg["Ly"], cfg["Lz"])
+    outs = []
+    for _ in range(3):
+        ud, vd, wd = u.cuda(), v.cuda(), w.cuda()
+        p = torch.empty_like(vd)
+        plan.project(ud, vd, wd, p)
+        torch.cuda.synchronize()
+        outs.append((ud, vd, wd, p))
+    for o in outs[1:]:
+        assert all(torch.equal(a, b) for a, b in zip(outs[0], o))
+    plan.destroy()
+
+
 def test_accumulate_mode_parity():
     """afid_plan_set_accumulate(1): p_out = p_in + phi (P:L91, P:L116 delta form); the velocities as before."""
     cfg = synth.config("C1", nx=40, ny=64, nz=128, grid="tanh", s=3.0)
