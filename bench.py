@@ -30,7 +30,10 @@ METRIC = "fp64 projection Mpoints/s at 1024x1536x1536; % of B200 HBM roofline"
 UNIT = "Mpoints/s"
 # algorithmic HBM bytes per grid point of each kernel: fp64, complex = 16 B per 2 points
 ALG_BYTES_PER_POINT = {"k_div_r2c": 32.0, "k_fft_y": 16.0, "k_solve_x": 16.0, "k_ifft_y": 16.0, "k_c2r_z": 16.0,
-                       "k_correct": 56.0, "k_c2r_correct": 64.0}
+                       "k_correct": 56.0,
+                       # plane-pipelined sweeps (afid_plan_set_pipeline): the intermediates B, D (and the re-read of p)
+                       # stay in L2, so a sweep's algorithmic HBM bytes are its end-to-end streams only
+                       "sweep_forward": 32.0, "sweep_inverse": 64.0}
 PATH_ALG_BYTES_PER_POINT = 96.0   # strict minimum of the whole path
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json north_star: "about 8 TB/s"
 
@@ -154,6 +157,11 @@ def run_gpu(args):
     N = nx * ny * nz
     xc = synth.grid_faces(cfg)
     plan = afid.Plan(nx, ny, nz, xc, cfg["Ly"], cfg["Lz"])
+    if args.pipeline:
+        pb, pr = (int(x) for x in args.pipeline.split(","))
+        plan.set_pipeline(pb, pr)
+    if args.hints is not None:
+        plan.set_l2_hints(args.hints)
     u = torch.empty((nx + 1, ny, nz), dtype=torch.float64, device=dev)
     v = torch.empty((nx, ny, nz), dtype=torch.float64, device=dev)
     w = torch.empty_like(v)
@@ -230,6 +238,9 @@ def run_gpu(args):
     # SURVEY.md 8(f) rows, timed outside the step: afid_max_cfl (24 B/pt) and afid_xsolve_apply (16 B/pt)
     extras = {}
     try:
+        if args.no_extras:
+            raise RuntimeError("skipped (--no-extras)")
+
         def timed(fn, reps=5):
             for _ in range(2):
                 fn()
@@ -342,6 +353,9 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--pipeline", default=None, help="planes_per_batch,rotation (afid_plan_set_pipeline)")
+    ap.add_argument("--hints", type=int, default=None, help="L2 hint mask (afid_plan_set_l2_hints)")
+    ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -119,6 +119,27 @@ afid_xsolve* afid_xsolve_create(afid_plan* plan, const double* a, const double* 
 int afid_xsolve_apply(afid_xsolve* h, double* f, void* stream);
 int afid_xsolve_destroy(afid_xsolve* h);
 
+/*
+ * afid_plan_set_pipeline -- run the two transform sweeps of afid_project plane-pipelined, so that their
+ * intermediates are handed from kernel to kernel inside the 126 MB L2 instead of through HBM (the paper's
+ * motivation for its hand-written local transposes, and for caring about bandwidth at all).
+ *   planes_per_batch > 0: the forward sweep (divergence + z transform, then y transform) and the inverse
+ *       sweep (inverse y transform, inverse z transform, correction) are launched in batches of that many
+ *       y-z planes on plan-owned streams, forked from and joined back to `stream` with events: the
+ *       kernels of batch b overlap those of batch b-1, and the z-transformed (y-transformed) plane goes
+ *       through a rotating buffer of `rotation` batches (2 <= rotation <= 7; planes_per_batch a multiple
+ *       of 2 where the inverse y transform handles two planes per CTA; planes_per_batch * rotation <= nx).
+ *   planes_per_batch <= 0: one launch per kernel over all planes (six launches; the default).
+ * Results are bit-identical in both modes.  Still capturable in a CUDA graph (fork/join by events).
+ * With timing enabled only the three sweeps are timed (afid_plan_num_timed).
+ * afid_plan_set_l2_hints -- bit mask of L2 eviction-priority hints the kernels attach to their accesses:
+ *   1 streamed loads (u, v, w, spectra read once) evict-first      2 intermediates (B, D) evict-last
+ *   4 loads of the intermediates evict-first                       8 streamed stores evict-first
+ * Default 0.  Hints change timing only, never results.
+ */
+int afid_plan_set_pipeline(afid_plan* plan, int planes_per_batch, int rotation);
+int afid_plan_set_l2_hints(afid_plan* plan, int mask);
+
 /* afid_plan_destroy -- free the plan's device and host memory.  NULL is a no-op.
  * The caller must have synchronised any stream still using the plan. */
 int afid_plan_destroy(afid_plan* plan);
@@ -134,9 +155,10 @@ int afid_plan_num_launches(const afid_plan* plan);
  * records a CUDA event on `stream` before and after each of its kernels (no host sync).
  * afid_plan_kernel_times synchronises on the last recorded event and writes the duration in
  * milliseconds of each kernel of the most recent afid_project call into ms[0..n-1]
- * (HOST pointer, n <= afid_plan_num_launches); afid_plan_kernel_name gives their names.
+ * (HOST pointer, n <= afid_plan_num_timed); afid_plan_kernel_name gives their names.
  */
 int afid_plan_enable_timing(afid_plan* plan, int on);
+int afid_plan_num_timed(const afid_plan* plan); /* entries afid_plan_kernel_times writes: 6 kernels, or 3 sweeps when pipelined */
 int afid_plan_kernel_times(afid_plan* plan, float* ms, int n);
 const char* afid_plan_kernel_name(const afid_plan* plan, int k);
 

@@ -24,7 +24,7 @@ SYMBOLS = ["afid_plan_create", "afid_project", "afid_plan_destroy", "afid_plan_w
            "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version",
            "afid_plan_enable_timing", "afid_plan_kernel_times", "afid_plan_kernel_name",
            "afid_fft_half_length_supported", "afid_max_cfl", "afid_plan_set_accumulate", "afid_xsolve_create", "afid_xsolve_apply",
-           "afid_xsolve_destroy"]
+           "afid_xsolve_destroy", "afid_plan_set_pipeline", "afid_plan_set_l2_hints", "afid_plan_num_timed"]
 
 _lib = None
 
@@ -80,6 +80,12 @@ def lib():
         L.afid_plan_enable_timing.argtypes = [vp, i]
         L.afid_plan_kernel_times.restype = i
         L.afid_plan_kernel_times.argtypes = [vp, vp, i]
+        L.afid_plan_set_pipeline.restype = i
+        L.afid_plan_set_pipeline.argtypes = [vp, i, i]
+        L.afid_plan_set_l2_hints.restype = i
+        L.afid_plan_set_l2_hints.argtypes = [vp, i]
+        L.afid_plan_num_timed.restype = i
+        L.afid_plan_num_timed.argtypes = [vp]
         L.afid_plan_kernel_name.restype = C.c_char_p
         L.afid_plan_kernel_name.argtypes = [vp, i]
         _lib = L
@@ -187,13 +193,21 @@ class Plan:
                                   _dev_ptr(w, n, "w"), _dev_ptr(out, 1, "cfl"), self._stream(stream)))
         return out
 
+    def set_pipeline(self, planes_per_batch, rotation=2):
+        """afid_plan_set_pipeline: plane-pipelined sweeps with L2-resident intermediates (0 = off)."""
+        _check(lib().afid_plan_set_pipeline(self._h, int(planes_per_batch), int(rotation)))
+
+    def set_l2_hints(self, mask):
+        """afid_plan_set_l2_hints: bit mask of L2 eviction-priority hints (timing only)."""
+        _check(lib().afid_plan_set_l2_hints(self._h, int(mask)))
+
     def enable_timing(self, on=True):
         """afid_plan_enable_timing: record CUDA events around each kernel of project()."""
         _check(lib().afid_plan_enable_timing(self._h, 1 if on else 0))
 
     def kernel_times(self):
         """afid_plan_kernel_times: {kernel name: ms} of the most recent project() (synchronises)."""
-        n = self.num_launches
+        n = int(lib().afid_plan_num_timed(self._h))
         ms = (C.c_float * n)()
         _check(lib().afid_plan_kernel_times(self._h, C.cast(ms, C.c_void_p), n))
         return {lib().afid_plan_kernel_name(self._h, k).decode(): float(ms[k]) for k in range(n)}

@@ -12,9 +12,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libafid_b200.so")
 SOURCES = ["afid_plan.cu"]
-HEADERS = ["afid_kernels.cuh", "fft_device.cuh", os.path.join("..", "..", "include", "afid.h")]
+import glob
+# every header the library is built from: editing any of them makes the built library stale
+HEADERS = sorted(os.path.basename(h) for h in glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join("..", "..", "include", "afid.h")]
+# only the afid_* entry points of include/afid.h are exported (-fvisibility=hidden + explicit default visibility)
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+              "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-shared", "-Xptxas", "-v"]
 
 
 def _stale():

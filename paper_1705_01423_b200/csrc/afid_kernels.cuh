@@ -73,35 +73,12 @@ __device__ __forceinline__ void stc_h(cplx* p, cplx v, unsigned long long pol)
 }
 
 __device__ __forceinline__ double2 ldg2(const double* p) { return __ldg(reinterpret_cast<const double2*>(p)); }
-// volatile read-only loads and a register "pin": see K1
-__device__ __forceinline__ double2 ldv2(const double* p)
-{
-    double2 r;
-    asm volatile("ld.global.nc.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
-    return r;
-}
-__device__ __forceinline__ double ldv1(const double* p)
-{
-    double r;
-    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(r) : "l"(p));
-    return r;
-}
+// a register "pin": see K1
 // scheduling fence between a load batch and its consumers; only the converged lanes take part
 // (the callers sit inside `if (act)`: a full-mask __syncwarp there would hang on partial warps)
 #define SCHED_FENCE() __syncwarp(__activemask())
 __device__ __forceinline__ void pin(double2& a) { asm volatile("" : "+d"(a.x), "+d"(a.y)); }
 __device__ __forceinline__ void pin1(double& a) { asm volatile("" : "+d"(a)); }
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
-{
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async16h(void* smem_dst, const void* gsrc, unsigned long long pol)
-{
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------
 // K1: divergence + r2c along z.  CTA = (i, group of NL consecutive j); NL*TPL threads.
@@ -400,191 +377,6 @@ __global__ void __launch_bounds__(LPR* PL::TPL, (LPR * PL::TPL <= 384) ? 2 : 1) 
             }
         }
         if constexpr (PL::NPASS > 1) fft_tail_passes_acc<PL, 1, false>(acc, tl, true, P.tw_zh, st_p);
-    }
-}
-
-// ------------------------------------------------------------------------------------------
-// K5+K6 fused: inverse c2r along z, p = phi, and the velocity correction in one kernel,
-// so that the transform of one CTA (compute) overlaps the u, v, w streaming of its SM neighbour (HBM), and
-// phi is corrected from shared memory instead of being read back.
-// Tile (i, jt) = 8 lines j0..j0+7 of plane i, as in k_c2r_z.  The correction also needs phi(i-1, same lines)
-// and phi(i, j0-1): both belong to tiles that were STARTED earlier (tiles are handed out in ticket order:
-// chunks of JC tiles outermost, then i, then the tile inside the chunk) and that publish "phi is in global
-// memory" through a per-tile flag before they wait for anything themselves -- so a wait can never deadlock.
-// Flags hold the epoch (the plan's call counter) and need no reset; the ticket wraps by atomicInc.
-// The periodic wrap v(i, 0) needs phi(i, ny-1): that line is corrected by the LAST tile of the plane.
-// ------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p)
-{
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v)
-{
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-__device__ __forceinline__ double2 ldcg2(const double* p)
-{
-    double2 r;
-    asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
-    return r;
-}
-constexpr int K56_JC = 4; // tiles per chunk (32 lines): phi(i-1) of a tile was written K56_JC tiles earlier
-
-template <class PL, int LPR>
-__global__ void __launch_bounds__(LPR* PL::TPL, (LPR * PL::TPL <= 384) ? 2 : 1)
-    k_c2r_correct(DevParams P, const __grid_constant__ CUtensorMap mapD, double* __restrict__ p, double* __restrict__ u, double* __restrict__ v,
-                  double* __restrict__ w, unsigned* __restrict__ sync, unsigned epoch)
-{
-    constexpr int Nh = PL::N, TPL = PL::TPL, NL = 8, NT = LPR * TPL, JC = K56_JC;
-    extern __shared__ __align__(1024) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t bar;
-    __shared__ unsigned s_ticket;
-    cplx* sm = reinterpret_cast<cplx*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u));
-    const int njt = P.ny / 8;
-    unsigned* flags = sync + 1;
-    if (threadIdx.x == 0) {
-        s_ticket = atomicInc(sync, gridDim.x - 1);
-        mbar_init(&bar, 1);
-        fence_mbar_init();
-    }
-    __syncthreads();
-    int i, jt;
-    {
-        const int t = (int)s_ticket, per_chunk = P.nx * JC;
-        const int chunk = t / per_chunk, rem = t % per_chunk;
-        const int jc_here = min(JC, njt - chunk * JC);
-        i = rem / jc_here;
-        jt = chunk * JC + rem % jc_here;
-    }
-    if (threadIdx.x == 0) {
-        constexpr int nb = k5_num_boxes(Nh), br = k5_box_rows(Nh);
-        const unsigned long long pol = l2_policy((P.hints & 4) ? 1 : ((P.hints & 2) ? 2 : 0));
-        mbar_expect_tx(&bar, (uint32_t)(nb * br * 8 * sizeof(cplx)));
-        for (int b = 0; b < nb; ++b) tma_load_3d_hint(sm + (size_t)b * br * 8, &mapD, jt * 16, b * br, i, &bar, pol);
-    }
-    auto at = [sm](int l, int r) -> cplx& { return sm[(r << 3) + (l ^ (r & 7))]; };
-    mbar_wait(&bar, 0);
-    for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NT) {
-        const int k = idx >> 3, l = idx & 7;
-        const int km = Nh - k;
-        const cplx xk = at(l, k);
-        const cplx xm = at(l, km);
-        const cplx wk = __ldg(&P.tw_z[k]);
-        const cplx E = mk(xk.x + xm.x, xk.y - xm.y), O = mk(xk.x - xm.x, xk.y + xm.y);
-        const cplx wo = mk(fma(wk.y, O.y, wk.x * O.x), fma(-wk.y, O.x, wk.x * O.y)); // conj(w) * O
-        const cplx t = mk(-wo.y, wo.x);                                              // i conj(w) O
-        at(l, k) = mk(E.y + t.y, E.x + t.x);
-        if (k != 0 && k != km) at(l, km) = mk(-(E.y - t.y), E.x - t.x);
-    }
-    __syncthreads();
-    {   // the 8 transforms; the result stays in shared memory: slot pad(m) of line l = (phi(2m+1), phi(2m))
-        const int lr = threadIdx.x / TPL, tl = threadIdx.x % TPL;
-#pragma unroll 1
-        for (int rnd = 0; rnd < NL / LPR; ++rnd) {
-            const int ln = rnd * LPR + lr;
-            auto acc = [sm, ln](int pe) -> cplx& { return sm[(pe << 3) + (ln ^ (pe & 7))]; };
-            typedef FftPass<PL, 0> P0;
-            typename P0::Regs rg;
-            P0::load(rg, tl, [&](int e) { return at(ln, e); });
-            __syncthreads();
-            P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { acc(PL::pad(e)) = val; });
-            if constexpr (PL::NPASS > 1) fft_tail_passes_acc<PL, 1, true>(acc, tl, true, P.tw_zh, [](int, cplx) {});
-        }
-        __syncthreads();
-    }
-    auto phi2 = [sm](int l, int m) -> double2 { // (phi(2m), phi(2m+1)) of line l
-        const int pe = PL::pad(m);
-        const cplx z = sm[(pe << 3) + (l ^ (pe & 7))];
-        return make_double2(z.y, z.x);
-    };
-    const size_t plane = (size_t)P.ny * P.nz;
-    const size_t o0 = ((size_t)i * P.ny + (size_t)jt * 8) * P.nz; // first line of the tile
-    // 1. p = phi to global memory, then publish the tile
-    for (int idx = threadIdx.x; idx < NL * Nh; idx += NT) {
-        const int l = idx / Nh, m = idx % Nh;
-        *reinterpret_cast<double2*>(p + o0 + (size_t)l * P.nz + 2 * m) = phi2(l, m);
-    }
-    __threadfence();
-    __syncthreads();
-    const int tile = i * njt + jt;
-    if (threadIdx.x == 0) {
-        st_release_u32(&flags[tile], epoch);
-        // 2. wait for the tiles this one reads phi from (all started before this one)
-        //    (a bounded spin: a flag that never arrives is a bug and must trap, not hang the device)
-        auto wait_tile = [&](int t) {
-            for (unsigned n = 0; ld_acquire_u32(&flags[t]) != epoch; ++n) {
-                __nanosleep(64);
-                if (n > (1u << 25)) __trap();
-            }
-        };
-        if (i >= 1) wait_tile(tile - njt);
-        if (jt >= 1) wait_tile(tile - 1);
-        if (jt == njt - 1 && njt > 1) wait_tile(i * njt);
-    }
-    __syncthreads();
-    // 3. correction, line by line; every thread first issues the loads of all its pairs of the line
-    constexpr int NIT = (Nh + NT - 1) / NT;
-    const double rdy = P.rdy, rdz = P.rdz;
-    const bool has_u = (i >= 1);
-    const double rdc = has_u ? __ldg(&P.rdc[i]) : 0.0;
-    const unsigned long long pol_in = l2_policy((P.hints & 1) ? 1 : 0), pol_out = l2_policy((P.hints & 8) ? 1 : 0);
-#pragma unroll 1
-    for (int l = 0; l < NL; ++l) {
-        const size_t ol = o0 + (size_t)l * P.nz;
-        // line j-1: in shared memory, except for the first line of the tile (left neighbour tile / deferred wrap)
-        const bool pj_smem = (l >= 1) || (njt == 1);
-        const bool do_v = pj_smem || (jt >= 1);
-        const double* pj_g = p + ol - P.nz; // only used when !pj_smem && do_v
-        const int lj = (l >= 1) ? l - 1 : NL - 1;
-        double2 uu[NIT], vv[NIT], ww[NIT], pi[NIT], pjg[NIT];
-#pragma unroll
-        for (int r = 0; r < NIT; ++r) {
-            const int m = threadIdx.x + r * NT;
-            if (m < Nh) {
-                ww[r] = ldc_h(reinterpret_cast<const cplx*>(w + ol + 2 * m), pol_in);
-                if (do_v) vv[r] = ldc_h(reinterpret_cast<const cplx*>(v + ol + 2 * m), pol_in);
-                if (do_v && !pj_smem) pjg[r] = ldcg2(pj_g + 2 * m);
-                if (has_u) {
-                    uu[r] = ldc_h(reinterpret_cast<const cplx*>(u + ol + 2 * m), pol_in);
-                    pi[r] = ldcg2(p + ol - plane + 2 * m);
-                }
-            }
-        }
-#pragma unroll
-        for (int r = 0; r < NIT; ++r) {
-            const int m = threadIdx.x + r * NT;
-            if (m < Nh) {
-                const double2 ph = phi2(l, m);
-                const double pk = phi2(l, m == 0 ? Nh - 1 : m - 1).y;
-                ww[r].x -= (ph.x - pk) * rdz;
-                ww[r].y -= (ph.y - ph.x) * rdz;
-                stc_h(reinterpret_cast<cplx*>(w + ol + 2 * m), ww[r], pol_out);
-                if (do_v) {
-                    const double2 pj = pj_smem ? phi2(lj, m) : pjg[r];
-                    vv[r].x -= (ph.x - pj.x) * rdy;
-                    vv[r].y -= (ph.y - pj.y) * rdy;
-                    stc_h(reinterpret_cast<cplx*>(v + ol + 2 * m), vv[r], pol_out);
-                }
-                if (has_u) {
-                    uu[r].x -= (ph.x - pi[r].x) * rdc;
-                    uu[r].y -= (ph.y - pi[r].y) * rdc;
-                    stc_h(reinterpret_cast<cplx*>(u + ol + 2 * m), uu[r], pol_out);
-                }
-            }
-        }
-    }
-    if (jt == njt - 1 && njt > 1) { // the periodic wrap: v(i, 0) with phi(i, ny-1) = this tile's last line
-        const size_t og = (size_t)i * P.ny * P.nz;
-        for (int m = threadIdx.x; m < Nh; m += NT) {
-            const double2 ph = ldcg2(p + og + 2 * m);
-            const double2 pj = phi2(NL - 1, m);
-            double2 vv = ldc_h(reinterpret_cast<const cplx*>(v + og + 2 * m), pol_in);
-            vv.x -= (ph.x - pj.x) * rdy;
-            vv.y -= (ph.y - pj.y) * rdy;
-            stc_h(reinterpret_cast<cplx*>(v + og + 2 * m), vv, pol_out);
-        }
     }
 }
 
@@ -1068,15 +860,22 @@ __global__ void __launch_bounds__(64 * KW, (KW == 4) ? 3 : 1) k_xsolve_field(Dev
 //   cflm = max(1e-8, max over cells 0.5 (|w(k)+w(k+1)|/dz + |v(j)+v(j+1)|/dy + |u(i)+u(i+1)|/dx_i))
 // (AFiD's dz, dy, udx3m are inverse spacings).  Same CTA map as K6: (i, 4 lines), four 16-byte pairs per
 // thread per batch; plane i+1 of u and line j+1 of v are L2 hits.  Non-negative doubles order like
-// their bit patterns, so the grid-wide maximum is one atomicMax on the 64-bit pattern per CTA.
+// their bit patterns, so the grid-wide maximum is one atomicMax on the 64-bit pattern per CTA.  The whole
+// reduction runs on the bit patterns: a NaN (from a blown-up field) has the largest pattern and therefore
+// reaches the result instead of being dropped by fmax (a time stepper must see it).
 // ------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long cfl_bits(double q)   // q >= 0 or NaN
+{
+    return (unsigned long long)__double_as_longlong(q) & 0x7FFFFFFFFFFFFFFFull;
+}
+__device__ __forceinline__ unsigned long long umax64(unsigned long long a, unsigned long long b) { return a > b ? a : b; }
 __global__ void k_cfl_init(double* __restrict__ cfl) { *cfl = 0.00000001; }
 
 __global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const double* __restrict__ u, const double* __restrict__ v,
                                                           const double* __restrict__ w, double* __restrict__ cfl)
 {
     constexpr int JL = K6_JL, TX = K6_TX, U = K6_U;
-    __shared__ double s_max[JL * TX / 32];
+    __shared__ unsigned long long s_max[JL * TX / 32];
     const int ngrp = P.ny / JL;
     constexpr int JC = 32 / JL;
     const int per_chunk = P.nx * JC;
@@ -1095,7 +894,7 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const dou
     const double* vp = v + ((size_t)i * P.ny + jp) * P.nz;
     const int nzh2 = P.nz / 2;
     const double rdx = __ldg(&P.rdx[i]), rdy = P.rdy, rdz = P.rdz;
-    double best = 0.0;
+    unsigned long long best = 0ull;
     for (int k0 = threadIdx.x; k0 < nzh2; k0 += TX * U) {
         double2 u0[U], u1[U], v0[U], v1[U], w0[U];
         double wn[U];
@@ -1117,18 +916,18 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const dou
             if (kp < nzh2) {
                 const double qa = fabs((w0[r].x + w0[r].y) * rdz) + fabs((v0[r].x + v1[r].x) * rdy) + fabs((u0[r].x + u1[r].x) * rdx);
                 const double qb = fabs((w0[r].y + wn[r]) * rdz) + fabs((v0[r].y + v1[r].y) * rdy) + fabs((u0[r].y + u1[r].y) * rdx);
-                best = fmax(best, fmax(qa, qb) * 0.5);
+                best = umax64(best, umax64(cfl_bits(qa * 0.5), cfl_bits(qb * 0.5)));
             }
         }
     }
 #pragma unroll
-    for (int d = 16; d >= 1; d >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, d));
+    for (int d = 16; d >= 1; d >>= 1) best = umax64(best, __shfl_xor_sync(0xffffffffu, best, d));
     const int tid = threadIdx.y * TX + threadIdx.x;
     if ((tid & 31) == 0) s_max[tid >> 5] = best;
     __syncthreads();
     if (tid == 0) {
-        for (int k = 1; k < JL * TX / 32; ++k) best = fmax(best, s_max[k]);
-        atomicMax(reinterpret_cast<unsigned long long*>(cfl), (unsigned long long)__double_as_longlong(best));
+        for (int k = 1; k < JL * TX / 32; ++k) best = umax64(best, s_max[k]);
+        atomicMax(reinterpret_cast<unsigned long long*>(cfl), best);
     }
 }
 

@@ -105,10 +105,6 @@ template <class PL> LaunchCfg cfg_k4()
 {
     return {(const void*)k_ifft_y<PL, ky_nl<PL>()>, ky_nl<PL>() * tpl8<PL>(), (size_t)ky_nl<PL>() * PL::LS * sizeof(cplx), 3, ky_nl<PL>()};
 }
-template <class PL> LaunchCfg cfg_k56()
-{
-    return {(const void*)k_c2r_correct<PL, K5_LPR>, K5_LPR * PL::TPL, (size_t)k5_smem_rows<PL>() * 8 * sizeof(cplx) + 1024, 2};
-}
 template <class PL> LaunchCfg cfg_k5()
 {
     return {(const void*)k_c2r_z<PL, K5_LPR>, K5_LPR * PL::TPL, (size_t)k5_smem_rows<PL>() * 8 * sizeof(cplx) + 1024, 2};
@@ -130,7 +126,7 @@ bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4)
         return false;
     }
 }
-bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5, LaunchCfg* k56)
+bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5)
 {
     switch (n) {
 #define X(N, R0, R1, R2, R3, TPL)                   \
@@ -138,7 +134,6 @@ bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5, LaunchCfg* k56)
         typedef FftPlan<R0, R1, R2, R3, TPL> PL;    \
         if (k1) *k1 = cfg_k1<PL>();                 \
         if (k5) *k5 = cfg_k5<PL>();                 \
-        if (k56) *k56 = cfg_k56<PL>();              \
         return true;                                \
     }
         AFID_FFT_SIZES_Z(X)
@@ -162,7 +157,6 @@ LaunchCfg select_k3(int nx, int* kw_out)
         const size_t smem8 = (size_t)k3_tile_rows(nx) * 8 * sizeof(cplx) + (size_t)10 * ((nx + 15) / 16) * 8 * sizeof(double)
                              + (size_t)k3_coef_slots(nx, 16) * sizeof(double2) + 128;
         if (2 * (smem8 + 1024) > 228 * 1024) kw = 4;
-        if (getenv("AFID_K3_KW") && nx <= 1024) kw = atoi(getenv("AFID_K3_KW")) == 4 ? 4 : 8;
         const bool ex = (nx % 16 == 0);
         if (kw == 8) c.fn = ex ? (const void*)k_solve_x<16, true, 8, 512> : (const void*)k_solve_x<16, false, 8, 512>;
         else if (nx <= 1024) c.fn = ex ? (const void*)k_solve_x<16, true, 4, 256> : (const void*)k_solve_x<16, false, 4, 256>;
@@ -211,22 +205,30 @@ bool make_map3(CUtensorMap* m, void* base, uint64_t d0, uint64_t d1, uint64_t d2
 
 } // namespace
 
+// the auxiliary streams / events of the plane-pipelined sweeps (afid_plan_set_pipeline)
+constexpr int PIPE_STREAMS = 3;
+constexpr int PIPE_EVENTS = 8;   // per kind; >= the largest rotation depth + 1
+
 struct afid_plan {
     int nx, ny, nz, nzh;
+    int device;        // the device the plan was created on (its work arrays and tensor maps live there)
     DevParams dp;
     void* tables;      // one device allocation holding all tables
     size_t tables_bytes;
     cplx* ws[2];       // work arrays, nx*nzh*ny complex each
     size_t ws_bytes;
-    LaunchCfg k1, k2, k4, k5, k56, k3;
+    LaunchCfg k1, k2, k4, k5, k3;
     bool accumulate;   // p += phi instead of p = phi (afid_plan_set_accumulate)
-    bool fuse56;       // K5 and K6 as one kernel (k_c2r_correct) with inter-CTA flags
-    unsigned* sync56;  // ticket + one flag per tile (device)
-    unsigned epoch;    // call counter: the value the flags of the current call take
     int k3_kw;         // systems per K3 CTA (8 or 4)
     alignas(64) CUtensorMap mapC;   // K3's gather of C = ws[1] viewed as [nzh][nx][2 ny] doubles
     alignas(64) CUtensorMap mapD;   // K5's gather of D = ws[1], same view, 128-byte swizzle
     int n_sm;
+    // plane-pipelined sweeps (afid_plan_set_pipeline): batches of pipe_batch planes, intermediates B and D in
+    // a rotating buffer of pipe_rot batches that stays in L2
+    int pipe_batch, pipe_rot;
+    cudaStream_t aux[PIPE_STREAMS];
+    cudaEvent_t ev_fork, ev_join[PIPE_STREAMS], ev_a[PIPE_EVENTS], ev_b[PIPE_EVENTS];
+    bool pipe_ready;
     // optional per-kernel timing (afid_plan_enable_timing): NK+1 events around the NK kernels
     bool timing;
     cudaEvent_t ev[7];
@@ -234,47 +236,71 @@ struct afid_plan {
 };
 
 static const char* const KERNEL_NAMES[6] = {"k_div_r2c", "k_fft_y", "k_solve_x", "k_ifft_y", "k_c2r_z", "k_correct"};
-static const char* const KERNEL_NAMES_FUSED[5] = {"k_div_r2c", "k_fft_y", "k_solve_x", "k_ifft_y", "k_c2r_correct"};
-static bool fused_path(const afid_plan* pl) { return pl->fuse56; }
+// pipelined: the kernels of a sweep overlap, so only the three sweeps can be timed
+static const char* const SWEEP_NAMES[3] = {"sweep_forward", "k_solve_x", "sweep_inverse"};
+static bool pipelined(const afid_plan* pl) { return pl->pipe_batch > 0; }
+
+#define AFID_EXPORT __attribute__((visibility("default")))
 
 extern "C" {
 
-const char* afid_version(void) { return "afid-project-b200 0.1 (sm_100a, fp64)"; }
-const char* afid_last_error(void) { return g_err.c_str(); }
-int afid_last_error_code(void) { return g_err_code; }
-int afid_max_nx(void) { return MAX_NX; }
-int afid_fft_length_supported(int n) { return lookup_fft_y(n, nullptr, nullptr) ? 1 : 0; }
-int afid_fft_half_length_supported(int n) { return lookup_fft_z(n, nullptr, nullptr, nullptr) ? 1 : 0; }
+AFID_EXPORT const char* afid_version(void) { return "afid-project-b200 0.2 (sm_100a, fp64)"; }
+AFID_EXPORT const char* afid_last_error(void) { return g_err.c_str(); }
+AFID_EXPORT int afid_last_error_code(void) { return g_err_code; }
+AFID_EXPORT int afid_max_nx(void) { return MAX_NX; }
+AFID_EXPORT int afid_fft_length_supported(int n) { return lookup_fft_y(n, nullptr, nullptr) ? 1 : 0; }
+AFID_EXPORT int afid_fft_half_length_supported(int n) { return lookup_fft_z(n, nullptr, nullptr) ? 1 : 0; }
 
-static int set_smem_attr(const LaunchCfg& c)
+} // extern "C"
+
+// One kernel instantiation serves many grid sizes (and several live plans), so the dynamic shared-memory
+// limit of a function is raised to the device maximum once and never lowered; the carveout is a hint only.
+static int set_smem_attr(const LaunchCfg& c, size_t optin_max)
 {
-    // ask for the largest shared-memory carveout so that several CTAs fit per SM
     {
         const size_t per_sm = 228 * 1024;
         size_t want = (size_t)c.ctas_per_sm * (c.smem + 1024);
         if (want > per_sm) want = per_sm;
-        int pct = (int)((want * 100 + per_sm - 1) / per_sm);
-        if (getenv("AFID_CARVEOUT")) pct = atoi(getenv("AFID_CARVEOUT"));
-        if (pct >= 0) cudaFuncSetAttribute(c.fn, cudaFuncAttributePreferredSharedMemoryCarveout, pct);
+        const int pct = (int)((want * 100 + per_sm - 1) / per_sm);
+        cudaFuncSetAttribute(c.fn, cudaFuncAttributePreferredSharedMemoryCarveout, pct);
     }
-    if (c.smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(c.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
-        if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
-    }
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, c.fn);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaFuncGetAttributes: ") + cudaGetErrorString(e));
+    if (c.smem + fa.sharedSizeBytes > optin_max) return fail(AFID_ERR_UNSUPPORTED_SIZE, "tile does not fit shared memory");
+    e = cudaFuncSetAttribute(c.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(optin_max - fa.sharedSizeBytes));
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
     return AFID_OK;
+}
+
+static void destroy_pipeline(afid_plan* pl)
+{
+    if (!pl->pipe_ready) return;
+    cudaEventDestroy(pl->ev_fork);
+    for (int k = 0; k < PIPE_STREAMS; ++k) {
+        cudaStreamDestroy(pl->aux[k]);
+        cudaEventDestroy(pl->ev_join[k]);
+    }
+    for (int k = 0; k < PIPE_EVENTS; ++k) {
+        cudaEventDestroy(pl->ev_a[k]);
+        cudaEventDestroy(pl->ev_b[k]);
+    }
+    pl->pipe_ready = false;
 }
 
 // free whatever a partially built plan holds (the struct is zero-initialised; cudaFree(nullptr) is a no-op)
 static void discard_plan(afid_plan* pl)
 {
+    destroy_pipeline(pl);
     cudaFree(pl->ws[0]);
     cudaFree(pl->ws[1]);
     cudaFree(pl->tables);
-    cudaFree(pl->sync56);
     delete pl;
 }
 
-afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly, double Lz)
+extern "C" {
+
+AFID_EXPORT afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly, double Lz)
 {
     g_err.clear();
     g_err_code = 0;
@@ -289,7 +315,7 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     if (!pl) { fail(AFID_ERR_NOMEM, "host allocation failed"); return nullptr; }
     std::memset(pl, 0, sizeof(*pl));
     if (!lookup_fft_y(ny, &pl->k2, &pl->k4)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "ny is not a supported FFT length"); return nullptr; }
-    if (!lookup_fft_z(nh, &pl->k1, &pl->k5, &pl->k56)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "nz/2 is not a supported FFT length"); return nullptr; }
+    if (!lookup_fft_z(nh, &pl->k1, &pl->k5)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "nz/2 is not a supported FFT length"); return nullptr; }
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
 
     // ---- K3 configuration
@@ -301,10 +327,11 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
         delete pl; fail(AFID_ERR_CUDA, "no CUDA device"); return nullptr;
     }
     if (prop.major != 10) { delete pl; fail(AFID_ERR_CUDA, "this library is built for sm_100a (B200) only"); return nullptr; }
+    pl->device = dev;
     pl->n_sm = prop.multiProcessorCount;
-    for (const LaunchCfg* c : {&pl->k1, &pl->k2, &pl->k3, &pl->k4, &pl->k5, &pl->k56}) {
+    for (const LaunchCfg* c : {&pl->k1, &pl->k2, &pl->k3, &pl->k4, &pl->k5}) {
         if (c->smem > prop.sharedMemPerBlockOptin) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "tile does not fit shared memory"); return nullptr; }
-        if (set_smem_attr(*c) != AFID_OK) { delete pl; return nullptr; }
+        if (set_smem_attr(*c, prop.sharedMemPerBlockOptin) != AFID_OK) { delete pl; return nullptr; }
     }
 
     // ---- host tables (long double, rounded once to fp64)
@@ -328,7 +355,6 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     std::vector<double> twy(2 * (size_t)ny), twzh(2 * (size_t)nh), twz(2 * (size_t)(nh + 1));
     auto fill_tw = [&](std::vector<double>& t, int count, int n) {
         for (int k = 0; k < count; ++k) {
-            // reduce to the first octant for accuracy
             const ld ang = 2.0L * pi * (ld)k / (ld)n;
             t[2 * k] = (double)cosl(ang);
             t[2 * k + 1] = (double)(-sinl(ang));
@@ -353,13 +379,6 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
         if (cudaMemcpy((char*)pl->tables + it.off, it.src, it.bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
             discard_plan(pl); fail(AFID_ERR_CUDA, "cudaMemcpy(tables) failed"); return nullptr;
         }
-    pl->fuse56 = getenv("AFID_FUSE56") && atoi(getenv("AFID_FUSE56")) == 1; // off by default: slower than K5 + K6
-    {
-        const size_t nflag = 1 + (size_t)nx * (ny / 8);
-        if (cudaMalloc((void**)&pl->sync56, nflag * sizeof(unsigned)) != cudaSuccess || cudaMemset(pl->sync56, 0, nflag * sizeof(unsigned)) != cudaSuccess) {
-            cudaGetLastError(); discard_plan(pl); fail(AFID_ERR_NOMEM, "cudaMalloc(flags) failed"); return nullptr;
-        }
-    }
     pl->ws_bytes = (size_t)nx * pl->nzh * ny * sizeof(cplx);
     for (int b = 0; b < 2; ++b)
         if (cudaMalloc((void**)&pl->ws[b], pl->ws_bytes) != cudaSuccess) {
@@ -393,25 +412,59 @@ afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly,
     d.tw_zh = (const cplx*)(tb + items[8].off);
     d.tw_z = (const cplx*)(tb + items[9].off);
     d.inv_vol = (double)(1.0L / vol);
-    d.hints = getenv("AFID_HINTS") ? atoi(getenv("AFID_HINTS")) : 0;
+    d.hints = 0;
     return pl;
 }
 
-int afid_plan_destroy(afid_plan* pl)
+AFID_EXPORT int afid_plan_destroy(afid_plan* pl)
 {
     if (!pl) return AFID_OK;
     if (pl->timing)
         for (int k = 0; k < 7; ++k) cudaEventDestroy(pl->ev[k]);
-    cudaFree(pl->ws[0]);
-    cudaFree(pl->ws[1]);
-    cudaFree(pl->tables);
-    cudaFree(pl->sync56);
-    delete pl;
+    discard_plan(pl);
     return AFID_OK;
 }
 
-size_t afid_plan_workspace_bytes(const afid_plan* pl) { return pl ? 2 * pl->ws_bytes + pl->tables_bytes : 0; }
-int afid_plan_num_launches(const afid_plan* pl) { return pl ? (fused_path(pl) ? 5 : 6) : 0; }
+AFID_EXPORT size_t afid_plan_workspace_bytes(const afid_plan* pl) { return pl ? 2 * pl->ws_bytes + pl->tables_bytes : 0; }
+
+AFID_EXPORT int afid_plan_num_launches(const afid_plan* pl)
+{
+    if (!pl) return 0;
+    if (!pipelined(pl)) return 6;
+    const int nb = (pl->nx + pl->pipe_batch - 1) / pl->pipe_batch;
+    return 5 * nb + 1;
+}
+
+AFID_EXPORT int afid_plan_set_l2_hints(afid_plan* pl, int mask)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    if (mask < 0 || mask > 15) return fail(AFID_ERR_UNSUPPORTED_SIZE, "hint mask must be in [0, 15]");
+    pl->dp.hints = mask;
+    return AFID_OK;
+}
+
+AFID_EXPORT int afid_plan_set_pipeline(afid_plan* pl, int planes_per_batch, int rotation)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    if (planes_per_batch <= 0) { pl->pipe_batch = 0; pl->pipe_rot = 0; return AFID_OK; }
+    if (rotation < 2 || rotation >= PIPE_EVENTS) return fail(AFID_ERR_UNSUPPORTED_SIZE, "rotation must be in [2, 7]");
+    if ((planes_per_batch % pl->k4.nl) != 0) return fail(AFID_ERR_UNSUPPORTED_SIZE, "planes_per_batch must be a multiple of the planes one inverse-transform CTA handles");
+    if ((size_t)planes_per_batch * rotation > (size_t)pl->nx) return fail(AFID_ERR_UNSUPPORTED_SIZE, "planes_per_batch * rotation exceeds nx");
+    if (!pl->pipe_ready) {
+        bool ok = cudaEventCreateWithFlags(&pl->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+        for (int k = 0; k < PIPE_STREAMS && ok; ++k)
+            ok = cudaStreamCreateWithFlags(&pl->aux[k], cudaStreamNonBlocking) == cudaSuccess && cudaEventCreateWithFlags(&pl->ev_join[k], cudaEventDisableTiming) == cudaSuccess;
+        for (int k = 0; k < PIPE_EVENTS && ok; ++k)
+            ok = cudaEventCreateWithFlags(&pl->ev_a[k], cudaEventDisableTiming) == cudaSuccess && cudaEventCreateWithFlags(&pl->ev_b[k], cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) return fail(AFID_ERR_CUDA, "stream / event creation failed");
+        pl->pipe_ready = true;
+    }
+    pl->pipe_batch = planes_per_batch;
+    pl->pipe_rot = rotation;
+    return AFID_OK;
+}
+
+} // extern "C"
 
 static int launch(const LaunchCfg& c, unsigned grid, cudaStream_t st, void** args, const char* name)
 {
@@ -427,20 +480,98 @@ static int check_ptr(const void* p, const char* name)
     return AFID_OK;
 }
 
+// the plan's work arrays, tables and tensor maps live on the device it was created on
+static int check_device(const afid_plan* pl)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaGetDevice failed");
+    if (dev != pl->device) return fail(AFID_ERR_CUDA, "the current device is not the device the plan was created on");
+    return AFID_OK;
+}
+
+static int record(cudaEvent_t ev, cudaStream_t st)
+{
+    cudaError_t e = cudaEventRecord(ev, st);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaEventRecord: ") + cudaGetErrorString(e));
+    return AFID_OK;
+}
+static int wait_on(cudaStream_t st, cudaEvent_t ev)
+{
+    cudaError_t e = cudaStreamWaitEvent(st, ev, 0);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaStreamWaitEvent: ") + cudaGetErrorString(e));
+    return AFID_OK;
+}
+
+static int launch_k1(afid_plan* pl, const double* u, const double* v, const double* w, cplx* B, int i_base, int np, int bmod, cudaStream_t st)
+{
+    void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&B, &i_base, &np, &bmod};
+    return launch(pl->k1, (unsigned)(np * (pl->ny / K1_NL)), st, args, "k_div_r2c");
+}
+static int launch_k2(afid_plan* pl, const cplx* B, cplx* C, int i_base, int np, int bmod, cudaStream_t st)
+{
+    const int ngrp2 = (pl->nzh + pl->k2.nl - 1) / pl->k2.nl;
+    void* args[] = {&pl->dp, (void*)&B, (void*)&C, &i_base, &bmod};
+    return launch(pl->k2, (unsigned)(np * ngrp2), st, args, "k_fft_y");
+}
+static int launch_k4(afid_plan* pl, const cplx* T, cplx* D, int i_base, int np, int dmod, cudaStream_t st)
+{
+    void* args[] = {&pl->dp, (void*)&T, (void*)&D, &i_base, &np, &dmod};
+    return launch(pl->k4, (unsigned)(pl->nzh * ((np + pl->k4.nl - 1) / pl->k4.nl)), st, args, "k_ifft_y");
+}
+static int launch_k5(afid_plan* pl, double* phi, int i_base, int np, int dmod, cudaStream_t st)
+{
+    void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&phi, &i_base, &dmod};
+    return launch(pl->k5, (unsigned)(np * (pl->ny / 8)), st, args, "k_c2r_z");
+}
+static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st, double* pacc)
+{
+    void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, &i_base, &np, (void*)&pacc};
+    cudaError_t e = cudaLaunchKernel((const void*)k_correct, dim3((unsigned)(np * (pl->ny / K6_JL))), dim3(K6_TX, K6_JL), args, 0, st);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_correct: ") + cudaGetErrorString(e));
+    return AFID_OK;
+}
+
+// fork the auxiliary streams off `st` / join them back (both capturable in a CUDA graph)
+static int pipe_fork(afid_plan* pl, cudaStream_t st, int ns)
+{
+    int rc;
+    if ((rc = record(pl->ev_fork, st))) return rc;
+    for (int k = 0; k < ns; ++k)
+        if ((rc = wait_on(pl->aux[k], pl->ev_fork))) return rc;
+    return AFID_OK;
+}
+static int pipe_join(afid_plan* pl, cudaStream_t st, int ns)
+{
+    int rc;
+    for (int k = 0; k < ns; ++k)
+        if ((rc = record(pl->ev_join[k], pl->aux[k])) || (rc = wait_on(st, pl->ev_join[k]))) return rc;
+    return AFID_OK;
+}
+
 // K1 + K2: u,v,w -> C layout spectrum in `outC`
 static int run_forward(afid_plan* pl, const double* u, const double* v, const double* w, cplx* wsB, cplx* outC, cudaStream_t st,
                        cudaEvent_t ev_mid)
 {
     int rc;
-    const int ngrp2 = (pl->nzh + pl->k2.nl - 1) / pl->k2.nl;
-    int i_base = 0, np = pl->nx, bmod = pl->nx;
-    {
-        void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&wsB, &i_base, &np, &bmod};
-        if ((rc = launch(pl->k1, (unsigned)(pl->nx * (pl->ny / K1_NL)), st, args, "k_div_r2c"))) return rc;
+    if (!pipelined(pl)) {
+        if ((rc = launch_k1(pl, u, v, w, wsB, 0, pl->nx, pl->nx, st))) return rc;
+        if (ev_mid && (rc = record(ev_mid, st))) return rc;
+        return launch_k2(pl, wsB, outC, 0, pl->nx, pl->nx, st);
     }
-    if (ev_mid) cudaEventRecord(ev_mid, st);
-    void* args[] = {&pl->dp, (void*)&wsB, (void*)&outC, &i_base, &bmod};
-    return launch(pl->k2, (unsigned)(pl->nx * ngrp2), st, args, "k_fft_y");
+    // plane-pipelined: K1 of batch b (stream 0) overlaps K2 of batch b-1 (stream 1); B is a rotating buffer of
+    // `rot` batches (the first planes of the work array), so that it is produced and consumed inside L2
+    const int nb = pl->pipe_batch, rot = pl->pipe_rot, bmod = nb * rot;
+    if ((rc = pipe_fork(pl, st, 2))) return rc;
+    int b = 0;
+    for (int i_base = 0; i_base < pl->nx; i_base += nb, ++b) {
+        const int np = (pl->nx - i_base < nb) ? pl->nx - i_base : nb;
+        if (b >= rot && (rc = wait_on(pl->aux[0], pl->ev_b[(b - rot) % PIPE_EVENTS]))) return rc;   // slot consumed
+        if ((rc = launch_k1(pl, u, v, w, wsB, i_base, np, bmod, pl->aux[0]))) return rc;
+        if ((rc = record(pl->ev_a[b % PIPE_EVENTS], pl->aux[0])) || (rc = wait_on(pl->aux[1], pl->ev_a[b % PIPE_EVENTS]))) return rc;
+        if ((rc = launch_k2(pl, wsB, outC, i_base, np, bmod, pl->aux[1]))) return rc;
+        if ((rc = record(pl->ev_b[b % PIPE_EVENTS], pl->aux[1]))) return rc;
+    }
+    return pipe_join(pl, st, 2);
 }
 
 // K3: C (always ws[1]: the tensor map is bound to it) -> T
@@ -450,66 +581,72 @@ static int run_solve(afid_plan* pl, cplx* outT, cudaStream_t st)
     return launch(pl->k3, (unsigned)(pl->nzh * (pl->ny / pl->k3_kw)), st, args, "k_solve_x");
 }
 
-static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st, double* pacc)
-{
-    void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, &i_base, &np, (void*)&pacc};
-    cudaError_t e = cudaLaunchKernel((const void*)k_correct, dim3((unsigned)(np * (pl->ny / K6_JL))), dim3(K6_TX, K6_JL), args, 0, st);
-    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_correct: ") + cudaGetErrorString(e));
-    return AFID_OK;
-}
-
-// K4 + K5 + K6 (or K4 + the fused K5/K6): T -> D -> p, u, v, w
+// K4 + K5 + K6: T -> D -> p, u, v, w
 static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double* v, double* w, double* p, cudaStream_t st,
                        cudaEvent_t ev_a, cudaEvent_t ev_b)
 {
     int rc;
-    int i_base = 0, np = pl->nx, dmod = pl->nx;
-    {
-        void* args[] = {&pl->dp, (void*)&T, (void*)&D, &i_base, &np, &dmod};
-        if ((rc = launch(pl->k4, (unsigned)(pl->nzh * ((pl->nx + pl->k4.nl - 1) / pl->k4.nl)), st, args, "k_ifft_y"))) return rc;
-    }
-    if (ev_a) cudaEventRecord(ev_a, st);
-    if (pl->fuse56) {
-        unsigned epoch = ++pl->epoch;
-        void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&p, (void*)&u, (void*)&v, (void*)&w, (void*)&pl->sync56, &epoch};
-        return launch(pl->k56, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_correct");
-    }
     // accumulate mode: phi goes to the (now dead) T work array, K6 corrects from it and adds it to p
     double* phi = pl->accumulate ? reinterpret_cast<double*>(pl->ws[0]) : p;
-    {
-        void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&phi, &i_base, &dmod};
-        if ((rc = launch(pl->k5, (unsigned)(pl->nx * (pl->ny / 8)), st, args, "k_c2r_z"))) return rc;
+    double* pacc = pl->accumulate ? p : nullptr;
+    if (!pipelined(pl) || pl->accumulate) {   // (accumulate: phi overwrites T plane by plane, which the pipelined K4 still reads)
+        if ((rc = launch_k4(pl, T, D, 0, pl->nx, pl->nx, st))) return rc;
+        if (ev_a && (rc = record(ev_a, st))) return rc;
+        if ((rc = launch_k5(pl, phi, 0, pl->nx, pl->nx, st))) return rc;
+        if (ev_b && (rc = record(ev_b, st))) return rc;
+        return launch_correct(pl, u, v, w, phi, 0, pl->nx, st, pacc);
     }
-    if (ev_b) cudaEventRecord(ev_b, st);
-    return launch_correct(pl, u, v, w, phi, 0, pl->nx, st, pl->accumulate ? p : nullptr);
+    // plane-pipelined: K4 of batch b (stream 0), K5 of batch b-1 (stream 1) and K6 of batch b-2 (stream 2)
+    // overlap; D is a rotating buffer of `rot` batches, p is read back by K6 right after K5 wrote it
+    const int nb = pl->pipe_batch, rot = pl->pipe_rot, dmod = nb * rot;
+    if ((rc = pipe_fork(pl, st, 3))) return rc;
+    int b = 0;
+    for (int i_base = 0; i_base < pl->nx; i_base += nb, ++b) {
+        const int np = (pl->nx - i_base < nb) ? pl->nx - i_base : nb;
+        if (b >= rot && (rc = wait_on(pl->aux[0], pl->ev_b[(b - rot) % PIPE_EVENTS]))) return rc;   // slot consumed
+        if ((rc = launch_k4(pl, T, D, i_base, np, dmod, pl->aux[0]))) return rc;
+        if ((rc = record(pl->ev_a[b % PIPE_EVENTS], pl->aux[0])) || (rc = wait_on(pl->aux[1], pl->ev_a[b % PIPE_EVENTS]))) return rc;
+        if ((rc = launch_k5(pl, phi, i_base, np, dmod, pl->aux[1]))) return rc;
+        // K6 of this batch also needs plane i_base-1 of phi: written by K5 of batch b-1, earlier on stream 1
+        if ((rc = record(pl->ev_b[b % PIPE_EVENTS], pl->aux[1])) || (rc = wait_on(pl->aux[2], pl->ev_b[b % PIPE_EVENTS]))) return rc;
+        if ((rc = launch_correct(pl, u, v, w, phi, i_base, np, pl->aux[2], pacc))) return rc;
+    }
+    return pipe_join(pl, st, 3);
 }
 
-int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void* stream)
+extern "C" {
+
+AFID_EXPORT int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void* stream)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     int rc;
     if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(p, "p"))) return rc;
+    if ((rc = check_device(pl))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const bool tm = pl->timing;
     cplx* wsB = pl->ws[0];
     cplx* wsC = pl->ws[1];
-    if (tm) cudaEventRecord(pl->ev[0], st);
+    if (tm && (rc = record(pl->ev[0], st))) return rc;
     if ((rc = run_forward(pl, u, v, w, wsB, wsC, st, tm ? pl->ev[1] : nullptr))) return rc;   // B in ws0, C in ws1
-    if (tm) cudaEventRecord(pl->ev[2], st);
+    if (tm && (rc = record(pl->ev[2], st))) return rc;
     if ((rc = run_solve(pl, pl->ws[0], st))) return rc;             // T in ws0
-    if (tm) cudaEventRecord(pl->ev[3], st);
+    if (tm && (rc = record(pl->ev[3], st))) return rc;
     if ((rc = run_inverse(pl, pl->ws[0], pl->ws[1], u, v, w, p, st, tm ? pl->ev[4] : nullptr, tm ? pl->ev[5] : nullptr))) return rc;
-    if (tm) { cudaEventRecord(pl->ev[6], st); pl->ev_valid = true; }
+    if (tm) {
+        if ((rc = record(pl->ev[6], st))) return rc;
+        pl->ev_valid = true;
+    }
     return AFID_OK;
 }
 
-int afid_max_cfl(afid_plan* pl, const double* u, const double* v, const double* w, double* cfl, void* stream)
+AFID_EXPORT int afid_max_cfl(afid_plan* pl, const double* u, const double* v, const double* w, double* cfl, void* stream)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     int rc;
     if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w"))) return rc;
     if (!cfl) return fail(AFID_ERR_NULL, "cfl is NULL");
     if (((size_t)cfl & 7) != 0) return fail(AFID_ERR_ALIGN, "cfl is not 8-byte aligned");
+    if ((rc = check_device(pl))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     k_cfl_init<<<1, 1, 0, st>>>(cfl);
     void* args[] = {&pl->dp, (void*)&u, (void*)&v, (void*)&w, (void*)&cfl};
@@ -518,10 +655,9 @@ int afid_max_cfl(afid_plan* pl, const double* u, const double* v, const double* 
     return AFID_OK;
 }
 
-int afid_plan_set_accumulate(afid_plan* pl, int on)
+AFID_EXPORT int afid_plan_set_accumulate(afid_plan* pl, int on)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
-    if (on && pl->fuse56) return fail(AFID_ERR_UNSUPPORTED_SIZE, "accumulate is not available on the fused K5/K6 path (AFID_FUSE56=1)");
     pl->accumulate = on != 0;
     return AFID_OK;
 }
@@ -533,9 +669,11 @@ struct afid_xsolve {
     LaunchCfg k;
     XsTables xt;       // device tables of the row-only quantities (k_xsolve_field)
     void* tables;      // one device allocation holding them
+    double* map_for;   // the field pointer `map` was encoded for (re-encoded only when it changes)
+    alignas(64) CUtensorMap map;
 };
 
-afid_xsolve* afid_xsolve_create(afid_plan* pl, const double* a_in, const double* c_in, const double* lam)
+AFID_EXPORT afid_xsolve* afid_xsolve_create(afid_plan* pl, const double* a_in, const double* c_in, const double* lam)
 {
     g_err.clear();
     g_err_code = 0;
@@ -559,7 +697,12 @@ afid_xsolve* afid_xsolve_create(afid_plan* pl, const double* a_in, const double*
     h->k.smem = (size_t)k3_tile_rows(nx) * KW * sizeof(cplx) + (size_t)2 * PCH * KW * sizeof(cplx) + 128;
     h->k.ctas_per_sm = 3;
     h->k.nl = KW;   // (complex lanes per tile)
-    if (set_smem_attr(h->k) != AFID_OK) { delete h; return nullptr; }
+    {
+        cudaDeviceProp prop;
+        if (cudaGetDeviceProperties(&prop, pl->device) != cudaSuccess) { delete h; fail(AFID_ERR_CUDA, "cudaGetDeviceProperties failed"); return nullptr; }
+        if (h->k.smem > prop.sharedMemPerBlockOptin) { delete h; fail(AFID_ERR_UNSUPPORTED_SIZE, "tile does not fit shared memory"); return nullptr; }
+        if (set_smem_attr(h->k, prop.sharedMemPerBlockOptin) != AFID_OK) { delete h; return nullptr; }
+    }
 
     // ---- the row-only quantities of the partitioned solve, in long double (same algebra as k_solve_x)
     typedef long double ld;
@@ -633,22 +776,25 @@ afid_xsolve* afid_xsolve_create(afid_plan* pl, const double* a_in, const double*
     return h;
 }
 
-int afid_xsolve_apply(afid_xsolve* h, double* f, void* stream)
+AFID_EXPORT int afid_xsolve_apply(afid_xsolve* h, double* f, void* stream)
 {
     if (!h) return fail(AFID_ERR_NULL, "xsolve handle is NULL");
     int rc;
     if ((rc = check_ptr(f, "f"))) return rc;
     const afid_plan* pl = h->pl;
-    alignas(64) CUtensorMap map;
-    if (!make_map3(&map, f, (uint64_t)pl->nz, (uint64_t)pl->ny, (uint64_t)pl->nx, 2 * (uint32_t)h->k.nl, 1, (uint32_t)k3_box_rows(pl->nx),
-                   CU_TENSOR_MAP_SWIZZLE_NONE))
-        return fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed");
+    if ((rc = check_device(pl))) return rc;
+    if (h->map_for != f) {
+        if (!make_map3(&h->map, f, (uint64_t)pl->nz, (uint64_t)pl->ny, (uint64_t)pl->nx, 2 * (uint32_t)h->k.nl, 1, (uint32_t)k3_box_rows(pl->nx),
+                       CU_TENSOR_MAP_SWIZZLE_NONE))
+            return fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed");
+        h->map_for = f;
+    }
     cplx* fc = reinterpret_cast<cplx*>(f);
-    void* args[] = {&h->dp, &h->xt, (void*)&map, (void*)&fc};
+    void* args[] = {&h->dp, &h->xt, (void*)&h->map, (void*)&fc};
     return launch(h->k, (unsigned)(pl->ny * ((pl->nz / 2) / h->k.nl)), (cudaStream_t)stream, args, "k_xsolve_field");
 }
 
-int afid_xsolve_destroy(afid_xsolve* h)
+AFID_EXPORT int afid_xsolve_destroy(afid_xsolve* h)
 {
     if (!h) return AFID_OK;
     cudaFree(h->tables);
@@ -656,7 +802,7 @@ int afid_xsolve_destroy(afid_xsolve* h)
     return AFID_OK;
 }
 
-int afid_plan_enable_timing(afid_plan* pl, int on)
+AFID_EXPORT int afid_plan_enable_timing(afid_plan* pl, int on)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     if (on && !pl->timing) {
@@ -672,25 +818,31 @@ int afid_plan_enable_timing(afid_plan* pl, int on)
     return AFID_OK;
 }
 
-int afid_plan_kernel_times(afid_plan* pl, float* ms, int n)
+AFID_EXPORT int afid_plan_kernel_times(afid_plan* pl, float* ms, int n)
 {
     if (!pl || !ms) return fail(AFID_ERR_NULL, "plan or ms is NULL");
     if (!pl->timing || !pl->ev_valid) return fail(AFID_ERR_CUDA, "timing not enabled or no projection recorded");
     if (cudaEventSynchronize(pl->ev[6]) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventSynchronize failed");
-    const int nk = fused_path(pl) ? 5 : 6;
-    for (int k = 0; k < nk && k < n; ++k) {
-        // fused path: the last kernel runs from ev[4] to ev[6] (ev[5] is not recorded)
-        cudaEvent_t e1 = (nk == 5 && k == 4) ? pl->ev[6] : pl->ev[k + 1];
-        if (cudaEventElapsedTime(&ms[k], pl->ev[k], e1) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventElapsedTime failed");
+    if (pipelined(pl)) {   // the kernels of a sweep overlap: forward sweep, x-solve, inverse sweep
+        const int a[3] = {0, 2, 3}, b[3] = {2, 3, 6};
+        for (int k = 0; k < 3 && k < n; ++k)
+            if (cudaEventElapsedTime(&ms[k], pl->ev[a[k]], pl->ev[b[k]]) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventElapsedTime failed");
+        return AFID_OK;
     }
+    for (int k = 0; k < 6 && k < n; ++k)
+        if (cudaEventElapsedTime(&ms[k], pl->ev[k], pl->ev[k + 1]) != cudaSuccess) return fail(AFID_ERR_CUDA, "cudaEventElapsedTime failed");
     return AFID_OK;
 }
 
-const char* afid_plan_kernel_name(const afid_plan* pl, int k)
+AFID_EXPORT int afid_plan_num_timed(const afid_plan* pl) { return pl ? (pipelined(pl) ? 3 : 6) : 0; }
+
+AFID_EXPORT const char* afid_plan_kernel_name(const afid_plan* pl, int k)
 {
-    if (pl && fused_path(pl)) return (k >= 0 && k < 5) ? KERNEL_NAMES_FUSED[k] : "";
+    if (pl && pipelined(pl)) return (k >= 0 && k < 3) ? SWEEP_NAMES[k] : "";
     return (k >= 0 && k < 6) ? KERNEL_NAMES[k] : "";
 }
+
+} // extern "C"
 
 // The taps speak [i][kz][ky]; the work array C is [kz][i][ky]: small re-layout kernels (not on the hot path).
 __global__ void k_tap_C_to_api(DevParams P, const cplx* __restrict__ C, cplx* __restrict__ A, int to_api)
@@ -716,7 +868,9 @@ __global__ void k_tap_T_to_api(DevParams P, const cplx* __restrict__ T, cplx* __
     }
 }
 
-int afid_stage_forward(afid_plan* pl, const double* u, const double* v, const double* w, double* spec, void* stream)
+extern "C" {
+
+AFID_EXPORT int afid_stage_forward(afid_plan* pl, const double* u, const double* v, const double* w, double* spec, void* stream)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     int rc;
@@ -729,7 +883,7 @@ int afid_stage_forward(afid_plan* pl, const double* u, const double* v, const do
     return AFID_OK;
 }
 
-int afid_stage_solve(afid_plan* pl, double* spec, void* stream)
+AFID_EXPORT int afid_stage_solve(afid_plan* pl, double* spec, void* stream)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     int rc;

@@ -101,20 +101,6 @@ def test_shapes_parity(ov):
     check_against_oracle(cfg, xc, u, v, w)
 
 
-@pytest.mark.parametrize("ov", [SHAPES[0], SHAPES[4], SHAPES[6], SHAPES[9]], ids=lambda o: f"{o['nx']}x{o['ny']}x{o['nz']}")
-def test_fused_c2r_correct_path(ov, monkeypatch):
-    """The alternative inverse path (K5 and K6 as one kernel with inter-CTA flags, AFID_FUSE56=1; off by
-    default) must give the same answer: one tile per plane (ny = 8, the periodic wrap
-    inside the tile), many tiles, a ragged chunk of tiles; two calls, so that the flag epoch advances."""
-    monkeypatch.setenv("AFID_FUSE56", "1")
-    cfg = synth.config("C1", **ov)
-    xc = synth.grid_faces(cfg)
-    u, v, w = synth.velocity(cfg, xc)
-    check_against_oracle(cfg, xc, u, v, w)
-    (u1, v1, w1, p1), (u2, v2, w2, p2) = gpu_project(cfg, xc, u, v, w, calls=2)
-    assert rel(u2, u1) <= 1e-11 and rel(v2, v1) <= 1e-11 and rel(w2, w1) <= 1e-11
-
-
 @pytest.mark.parametrize("ov", [SHAPES[1], SHAPES[4], SHAPES[7], dict(nx=256, ny=256, nz=256, grid="tanh", s=3.0)],
                          ids=lambda o: f"{o['nx']}x{o['ny']}x{o['nz']}")
 def test_max_cfl_parity(ov):
