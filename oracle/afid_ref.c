@@ -403,6 +403,48 @@ int afid_ref_project(int nx, int ny, int nz, const double *xc, double Ly, double
 }
 
 /* ------------------------------------------------------------------------------------
+ * Paper step 7 on a HALF spectrum [nx][ny][nz/2+1] (kz = 0..nz/2): the x-systems of the
+ * large-case oracle oracle/ref_dense.py, which keeps only the
+ * non-redundant half of the Hermitian spectrum of the real divergence.  Same long-double
+ * Thomas recurrences, same singular-mode handling as afid_ref_solve.  nz must be even.
+ * ---------------------------------------------------------------------------------- */
+int afid_ref_solve_half(int nx, int ny, int nz, const double *xc, double Ly, double Lz, double *hhat)
+{
+    if (nx < 2 || ny < 1 || nz < 2 || (nz & 1) || !xc || !hhat) return -1;
+    const int nzh = nz / 2 + 1;
+    double *dx = (double *)malloc(sizeof(double) * (size_t)nx);
+    double *dc = (double *)malloc(sizeof(double) * (size_t)(nx + 1));
+    double *ly = (double *)malloc(sizeof(double) * (size_t)ny);
+    double *lz = (double *)malloc(sizeof(double) * (size_t)nz);
+    ld *a = (ld *)malloc(sizeof(ld) * (size_t)nx), *c = (ld *)malloc(sizeof(ld) * (size_t)nx);
+    int rc = (!dx || !dc || !ly || !lz || !a || !c) ? -3 : afid_ref_metrics(nx, xc, dx, dc);
+    if (!rc) rc = afid_ref_wavenumbers(ny, Ly, ly);
+    if (!rc) rc = afid_ref_wavenumbers(nz, Lz, lz);
+    if (!rc) {
+        for (int i = 0; i < nx; ++i) {
+            a[i] = (i >= 1) ? 1.0L / ((ld)dx[i] * (ld)dc[i]) : 0.0L;
+            c[i] = (i <= nx - 2) ? 1.0L / ((ld)dx[i] * (ld)dc[i + 1]) : 0.0L;
+        }
+        const size_t stride = (size_t)ny * (size_t)nzh;
+#pragma omp parallel
+        {
+            ld *yr = (ld *)malloc(sizeof(ld) * (size_t)nx), *yi = (ld *)malloc(sizeof(ld) * (size_t)nx);
+            ld *g = (ld *)malloc(sizeof(ld) * (size_t)nx);
+#pragma omp for collapse(2) schedule(static)
+            for (int j = 0; j < ny; ++j)
+                for (int q = 0; q < nzh; ++q) {
+                    const ld lam = (ld)ly[j] + (ld)lz[q];
+                    solve_x_system(nx, a, c, dx, lam, (j == 0 && q == 0),
+                                   hhat + 2 * ((size_t)j * (size_t)nzh + (size_t)q), stride, yr, yi, g);
+                }
+            free(yr); free(yi); free(g);
+        }
+    }
+    free(dx); free(dc); free(ly); free(lz); free(a); free(c);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------
  * the maximum CFL number, the one routine the paper prints in full
  * (Listing 1 "CalcMaxCFL"):
  *     cflm = max( 1e-8, max over cells of

@@ -69,10 +69,13 @@ def divergence(xc, Ly, Lz, u, v, w):
     return d
 
 
-def correct(xc, Ly, Lz, phi, u, v, w):
-    """Returns corrected copies (u - G phi)."""
+def correct(xc, Ly, Lz, phi, u, v, w, inplace=False):
+    """Returns corrected copies (u - G phi); inplace=True updates the given contiguous fp64 arrays instead."""
     xc, phi = _f64(xc), _f64(phi)
-    u, v, w = _f64(u).copy(), _f64(v).copy(), _f64(w).copy()
+    if inplace:
+        assert all(isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous for a in (u, v, w))
+    else:
+        u, v, w = _f64(u).copy(), _f64(v).copy(), _f64(w).copy()
     nx, ny, nz = phi.shape
     _chk(lib().afid_ref_correct(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(xc), C.c_double(Ly),
                                 C.c_double(Lz), _p(phi), _p(u), _p(v), _p(w)), "afid_ref_correct")
@@ -128,6 +131,17 @@ def project(xc, Ly, Lz, u, v, w):
                                 C.c_double(Lz), _p(u), _p(v), _p(w), _p(p), C.byref(mi)),
          "afid_ref_project")
     return u, v, w, p, mi.value
+
+
+def solve_half(xc, Ly, Lz, nz, hhat):
+    """Per-mode x-solves IN PLACE on a half spectrum [nx][ny][nz/2+1] (complex128, C-contiguous)."""
+    xc = _f64(xc)
+    assert isinstance(hhat, np.ndarray) and hhat.dtype == np.complex128 and hhat.flags.c_contiguous
+    nx, ny, nzh = hhat.shape
+    assert nzh == nz // 2 + 1 and xc.size == nx + 1
+    _chk(lib().afid_ref_solve_half(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(xc), C.c_double(Ly),
+                                   C.c_double(Lz), _p(hhat)), "afid_ref_solve_half")
+    return hhat
 
 
 def max_cfl(xc, Ly, Lz, u, v, w):

@@ -334,6 +334,45 @@ def test_invariant_linearity_shift_mirror():
     np.testing.assert_allclose(mi[3], pa[3][::-1], atol=1e-12)
 
 
+def test_dense_large_case_oracle_matches_long_double_oracle():
+    """oracle/ref_dense.py (dense DFT matrices, fp64 matmuls, Hermitian fold in kz: the variant SURVEY.md 8(c) step 8
+    allows for C3 and larger) against the long-double definition, on non-power-of-two shapes, a non-uniform grid,
+    Ly != Lz, and on the mean-shear (C5-shaped) input; and against the manufactured Helmholtz answer (P2)."""
+    from oracle import ref_dense
+    for ov in (dict(nx=64, ny=96, nz=80, grid="tanh", s=3.0), dict(nx=9, ny=30, nz=36, grid="erf", s=1.5, x_lo=-1.0, x_hi=1.0,
+                                                                       Ly=3.0, Lz=0.7, shear=1.0, A=0.1)):
+        cfg = synth.config("C1", **ov)
+        xc = synth.grid_faces(cfg)
+        u, v, w = [t.numpy() for t in synth.velocity(cfg, xc)]
+        want = ref.project(xc, cfg["Ly"], cfg["Lz"], u, v, w)
+        uu, vv, ww = u.copy(), v.copy(), w.copy()
+        pp = ref_dense.project_dense(xc, cfg["Ly"], cfg["Lz"], uu, vv, ww)
+        for got, ref_ in zip((uu, vv, ww, pp), want[:4]):
+            assert rel(got, ref_) <= 1e-14
+        assert rel(uu - u, want[0] - u) <= 1e-13 and rel(vv - v, want[1] - v) <= 1e-13      # increments
+    # P2: u* = curl + G phi_m must come back as (curl, phi_m)
+    nx, ny, nz, Ly, Lz = 12, 10, 14, 1.3, 0.9
+    xc = tanh_grid(nx, 3.0)
+    dx, dc = ref.metrics(xc)
+    rng = np.random.default_rng(21)
+    dy, dz = Ly / ny, Lz / nz
+    psi = rng.standard_normal((nx, ny, nz))
+    chi = rng.standard_normal((nx + 1, ny, nz))
+    chi[0] = 0
+    chi[nx] = 0
+    u_s = (np.roll(chi, -1, axis=1) - chi) / dy
+    v_s = (np.roll(psi, -1, axis=2) - psi) / dz - (chi[1:] - chi[:-1]) / dx[:, None, None]
+    w_s = -(np.roll(psi, -1, axis=1) - psi) / dy
+    phi_m = rng.standard_normal((nx, ny, nz))
+    phi_m -= (phi_m * dx[:, None, None]).sum() / (dx.sum() * ny * nz)
+    uu = u_s.copy()
+    uu[1:nx] += (phi_m[1:] - phi_m[:-1]) / dc[1:nx, None, None]
+    vv = v_s + (phi_m - np.roll(phi_m, 1, axis=1)) / dy
+    ww = w_s + (phi_m - np.roll(phi_m, 1, axis=2)) / dz
+    pp = ref_dense.project_dense(xc, Ly, Lz, uu, vv, ww)
+    assert rel(pp, phi_m) <= 1e-12 and rel(uu, u_s) <= 1e-12 and rel(vv, v_s) <= 1e-12 and rel(ww, w_s) <= 1e-12
+
+
 def test_oracle_header_says_test_infrastructure():
     here = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     txt = open(os.path.join(here, "oracle", "afid_ref.c")).read()
