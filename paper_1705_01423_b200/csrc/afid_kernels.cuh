@@ -180,7 +180,16 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_
             P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { line[PL::pad(e)] = val; });
         }
     }
-    fft_tail_passes<PL, 1, true>(line, tl, true, P.tw_zh, [](int, cplx) {});
+    {   // barriers between the passes only over the warps of a line group (see K5); the split below needs all lines
+        constexpr int GL = (TPL % 32 == 0) ? 1 : ((2 * TPL) % 32 == 0 ? 2 : 4);
+        if constexpr (GL < NL && (GL * TPL) % 32 == 0) {
+            const GroupSync gsync{1 + ln / GL, GL * TPL};
+            fft_tail_passes_acc<PL, 1, true>([line](int pe) -> cplx& { return line[pe]; }, tl, true, P.tw_zh, [](int, cplx) {}, gsync);
+            __syncthreads();
+        } else {
+            fft_tail_passes<PL, 1, true>(line, tl, true, P.tw_zh, [](int, cplx) {});
+        }
+    }
 
     // split into the spectrum of the real line; thread -> (k, jl) with jl fastest
     const int jl0 = (jg * NL) % 8;         // position of this CTA's first line inside the tile
@@ -320,63 +329,93 @@ template <class PL> constexpr int k5_smem_rows()
     return tma_rows > fft_rows ? tma_rows : fft_rows;
 }
 
-template <class PL, int LPR>
-__global__ void __launch_bounds__(LPR* PL::TPL, (LPR * PL::TPL <= 384) ? 2 : 1) k_c2r_z(DevParams P, const __grid_constant__ CUtensorMap mapD, double* __restrict__ p, int i_base,
-                                                        int dmod)
+// Persistent: the launch has (at most) one CTA per SM (two for NBUF = 1), each walks over the tiles
+// t = blockIdx.x, blockIdx.x + gridDim.x, ... of planes i_base .. i_base+np-1.  With NBUF = 2 the tile of the next
+// step is gathered by TMA into the other buffer while this one is transformed, so HBM always has a request of
+// this SM in flight (the non-persistent version waited for its whole tile before doing anything: 17 % of its
+// stall samples).  A buffer is handed back to the async proxy (TMA writes) after a proxy fence and a CTA barrier.
+template <class PL, int LPR, int NBUF>
+__global__ void __launch_bounds__(LPR* PL::TPL, 1) k_c2r_z(DevParams P, const __grid_constant__ CUtensorMap mapD, double* __restrict__ p, int i_base, int np,
+                                                           int dmod)
 {
-    constexpr int Nh = PL::N, TPL = PL::TPL, NL = 8, NT = LPR * TPL;
+    constexpr int Nh = PL::N, TPL = PL::TPL, NL = 8;
+    constexpr int TILE = k5_smem_rows<PL>() * 8;     // complex slots per buffer
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t bar;
-    // 1024-byte aligned tile [row][8 chunks of 16 bytes]; line l, row r lives in chunk l ^ (r & 7)
+    __shared__ __align__(8) uint64_t bar[NBUF];
+    // 1024-byte aligned tiles [row][8 chunks of 16 bytes]; line l, row r lives in chunk l ^ (r & 7)
     // (the 128-byte TMA swizzle, kept for the in-place FFT passes: conflict-free for unit-stride rows)
-    cplx* sm = reinterpret_cast<cplx*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u)); // (offset form keeps the shared state space)
+    cplx* sm0 = reinterpret_cast<cplx*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u)); // (offset form keeps the shared state space)
     const int njt = P.ny / 8;
-    const int i = i_base + blockIdx.x / njt, jt = blockIdx.x % njt;
+    const int ntile = np * njt;
     if (threadIdx.x == 0) {
-        mbar_init(&bar, 1);
+#pragma unroll
+        for (int b = 0; b < NBUF; ++b) mbar_init(&bar[b], 1);
         fence_mbar_init();
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
+    const unsigned long long pol = l2_policy((P.hints & 4) ? 1 : ((P.hints & 2) ? 2 : 0));
+    auto issue = [&](int t, int buf) {   // one thread: gather tile t into buffer buf
         constexpr int nb = k5_num_boxes(Nh), br = k5_box_rows(Nh);
-        const unsigned long long pol = l2_policy((P.hints & 4) ? 1 : ((P.hints & 2) ? 2 : 0));
-        mbar_expect_tx(&bar, (uint32_t)(nb * br * 8 * sizeof(cplx)));
-        for (int b = 0; b < nb; ++b) tma_load_3d_hint(sm + (size_t)b * br * 8, &mapD, jt * 16, b * br, i % dmod, &bar, pol);
-    }
-    auto at = [sm](int l, int r) -> cplx& { return sm[(r << 3) + (l ^ (r & 7))]; };
-    mbar_wait(&bar, 0);
-    // Hermitian pre-processing fused into the first pass's loads: element e of the complex line is
-    //   Z'(e) = (X(e) + conj X(Nh-e)) + i conj(w^e) (X(e) - conj X(Nh-e)),   w = exp(-2 pi i / nz),
-    // formed from rows k = min(e, Nh-e) and Nh-k (stored re/im-swapped: the inverse runs as a forward transform)
-    auto zprime = [&](int l, int e) -> cplx {
-        const int k = min(e, Nh - e), km = Nh - k;
-        const cplx xk = at(l, k);
-        const cplx xm = at(l, km);
-        const cplx wk = __ldg(&P.tw_z[k]);
-        const cplx E = mk(xk.x + xm.x, xk.y - xm.y), O = mk(xk.x - xm.x, xk.y + xm.y);
-        const cplx wo = mk(fma(wk.y, O.y, wk.x * O.x), fma(-wk.y, O.x, wk.x * O.y)); // conj(w) * O
-        const cplx t = mk(-wo.y, wo.x);                                              // i conj(w) O
-        return (e == k) ? mk(E.y + t.y, E.x + t.x) : mk(-(E.y - t.y), E.x - t.x);
+        const int i = i_base + t / njt, jt = t % njt;
+        mbar_expect_tx(&bar[buf], (uint32_t)(nb * br * 8 * sizeof(cplx)));
+        for (int b = 0; b < nb; ++b) tma_load_3d_hint(sm0 + (size_t)buf * TILE + (size_t)b * br * 8, &mapD, jt * 16, b * br, i % dmod, &bar[buf], pol);
     };
+    if (threadIdx.x == 0 && (int)blockIdx.x < ntile) issue(blockIdx.x, 0);
     const int lr = threadIdx.x / TPL, tl = threadIdx.x % TPL;
+    // The passes of different lines are independent: the barriers between them only span the warps of a line
+    // group (the fewest lines that fill whole warps), so that one group's barrier wait is another group's issue slot.
+    constexpr int GL = (TPL % 32 == 0) ? 1 : ((2 * TPL) % 32 == 0 ? 2 : ((4 * TPL) % 32 == 0 ? 4 : 8));   // lines per group
+    constexpr bool GROUPED = (GL < LPR) && (LPR / GL <= 8);
+    const GroupSync gsync{1 + lr / GL, GROUPED ? GL * TPL : LPR * TPL};
+    auto sync = [&]() {
+        if constexpr (GROUPED) gsync();
+        else __syncthreads();
+    };
+    int n = 0;
 #pragma unroll 1
-    for (int rnd = 0; rnd < NL / LPR; ++rnd) {
-        const int ln = rnd * LPR + lr;
-        double* dst = p + ((size_t)i * P.ny + (size_t)jt * 8 + ln) * (size_t)P.nz;
-        auto st_p = [&](int e, cplx val) { reinterpret_cast<double2*>(dst)[e] = cswap(val); };
-        auto acc = [sm, ln](int pe) -> cplx& { return sm[(pe << 3) + (ln ^ (pe & 7))]; };
-        typedef FftPass<PL, 0> P0;
-        {
-            typename P0::Regs rg;
-            P0::load(rg, tl, [&](int e) { return zprime(ln, e); });   // unpadded rows, as TMA delivered them
-            if constexpr (PL::NPASS == 1) {
-                P0::compute_store(rg, tl, P.tw_zh, st_p);
-            } else {
-                __syncthreads();
-                P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { acc(PL::pad(e)) = val; });
+    for (int t = blockIdx.x; t < ntile; t += gridDim.x, ++n) {
+        const int buf = (NBUF == 2) ? (n & 1) : 0;
+        if (NBUF == 2 && threadIdx.x == 0 && t + (int)gridDim.x < ntile) issue(t + gridDim.x, buf ^ 1);
+        cplx* sm = sm0 + (size_t)buf * TILE;
+        const int i = i_base + t / njt, jt = t % njt;
+        auto at = [sm](int l, int r) -> cplx& { return sm[(r << 3) + (l ^ (r & 7))]; };
+        mbar_wait(&bar[buf], (NBUF == 2) ? ((n >> 1) & 1) : (n & 1));
+        // Hermitian pre-processing fused into the first pass's loads: element e of the complex line is
+        //   Z'(e) = (X(e) + conj X(Nh-e)) + i conj(w^e) (X(e) - conj X(Nh-e)),   w = exp(-2 pi i / nz),
+        // formed from rows k = min(e, Nh-e) and Nh-k (stored re/im-swapped: the inverse runs as a forward transform)
+        auto zprime = [&](int l, int e) -> cplx {
+            const int k = min(e, Nh - e), km = Nh - k;
+            const cplx xk = at(l, k);
+            const cplx xm = at(l, km);
+            const cplx wk = __ldg(&P.tw_z[k]);
+            const cplx E = mk(xk.x + xm.x, xk.y - xm.y), O = mk(xk.x - xm.x, xk.y + xm.y);
+            const cplx wo = mk(fma(wk.y, O.y, wk.x * O.x), fma(-wk.y, O.x, wk.x * O.y)); // conj(w) * O
+            const cplx tt = mk(-wo.y, wo.x);                                             // i conj(w) O
+            return (e == k) ? mk(E.y + tt.y, E.x + tt.x) : mk(-(E.y - tt.y), E.x - tt.x);
+        };
+#pragma unroll 1
+        for (int rnd = 0; rnd < NL / LPR; ++rnd) {
+            const int ln = rnd * LPR + lr;
+            double* dst = p + ((size_t)i * P.ny + (size_t)jt * 8 + ln) * (size_t)P.nz;
+            auto st_p = [&](int e, cplx val) { reinterpret_cast<double2*>(dst)[e] = cswap(val); };
+            auto acc = [sm, ln](int pe) -> cplx& { return sm[(pe << 3) + (ln ^ (pe & 7))]; };
+            typedef FftPass<PL, 0> P0;
+            {
+                typename P0::Regs rg;
+                P0::load(rg, tl, [&](int e) { return zprime(ln, e); });   // unpadded rows, as TMA delivered them
+                if constexpr (PL::NPASS == 1) {
+                    P0::compute_store(rg, tl, P.tw_zh, st_p);
+                } else {
+                    sync();
+                    P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { acc(PL::pad(e)) = val; });
+                }
             }
+            if constexpr (PL::NPASS > 1) fft_tail_passes_acc<PL, 1, false>(acc, tl, true, P.tw_zh, st_p, sync);
         }
-        if constexpr (PL::NPASS > 1) fft_tail_passes_acc<PL, 1, false>(acc, tl, true, P.tw_zh, st_p);
+        // this buffer goes back to the TMA (async proxy) at the next step (NBUF = 1) or the one after (NBUF = 2)
+        fence_proxy_async();
+        __syncthreads();
+        if (NBUF == 1 && threadIdx.x == 0 && t + (int)gridDim.x < ntile) issue(t + gridDim.x, 0);
     }
 }
 

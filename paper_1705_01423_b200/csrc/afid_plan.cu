@@ -80,7 +80,6 @@ int fail(int code, const std::string& msg)
     X(640, 16, 8, 5, 1, 40)
 
 constexpr int K1_NL = 4; // lines per CTA in K1 (two CTAs fill one 128-byte row of B)
-constexpr int K5_LPR = 4; // lines per round in K5 (8 lines per CTA, 2 rounds)
 // lines per CTA in K2 / K4: 2 (256-byte gather segments), 1 for the longest lines (two 256-thread CTAs per SM
 // instead of one 512-thread CTA)
 template <class PL> constexpr int ky_nl() { return tpl8<PL>() >= 256 ? 1 : 2; }
@@ -105,9 +104,15 @@ template <class PL> LaunchCfg cfg_k4()
 {
     return {(const void*)k_ifft_y<PL, ky_nl<PL>()>, ky_nl<PL>() * tpl8<PL>(), (size_t)ky_nl<PL>() * PL::LS * sizeof(cplx), 3, ky_nl<PL>()};
 }
+// K5: all 8 lines of a tile in one round where that leaves >= 128 registers per thread, else two rounds of 4;
+// two tile buffers (TMA prefetch of the next tile) where they fit the 227 KB of an SM
+template <class PL> constexpr int k5_lpr() { return (8 * PL::TPL <= 512) ? 8 : 4; }
+template <class PL> constexpr int k5_nbuf() { return (2 * (size_t)k5_smem_rows<PL>() * 8 * sizeof(cplx) + 2048 <= 227 * 1024) ? 2 : 1; }
 template <class PL> LaunchCfg cfg_k5()
 {
-    return {(const void*)k_c2r_z<PL, K5_LPR>, K5_LPR * PL::TPL, (size_t)k5_smem_rows<PL>() * 8 * sizeof(cplx) + 1024, 2};
+    // .nl = CTAs per SM the launch is sized for
+    return {(const void*)k_c2r_z<PL, k5_lpr<PL>(), k5_nbuf<PL>()>, k5_lpr<PL>() * PL::TPL,
+            (size_t)k5_nbuf<PL>() * k5_smem_rows<PL>() * 8 * sizeof(cplx) + 1024, 1, 1};
 }
 
 bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4)
@@ -334,6 +339,14 @@ AFID_EXPORT afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc
         if (set_smem_attr(*c, prop.sharedMemPerBlockOptin) != AFID_OK) { delete pl; return nullptr; }
     }
 
+    {   // K5 is persistent: as many CTAs as are resident at once
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pl->k5.fn, pl->k5.threads, pl->k5.smem) != cudaSuccess || occ < 1) {
+            cudaGetLastError(); delete pl; fail(AFID_ERR_CUDA, "k_c2r_z does not fit an SM"); return nullptr;
+        }
+        pl->k5.nl = occ;
+    }
+
     // ---- host tables (long double, rounded once to fp64)
     typedef long double ld;
     std::vector<double> dx(nx), dc(nx + 1, 0.0), rdx(nx), rdc(nx + 1, 0.0), ca(nx, 0.0), cc(nx, 0.0), lamy(ny), lamz(nh + 1);
@@ -520,8 +533,9 @@ static int launch_k4(afid_plan* pl, const cplx* T, cplx* D, int i_base, int np, 
 }
 static int launch_k5(afid_plan* pl, double* phi, int i_base, int np, int dmod, cudaStream_t st)
 {
-    void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&phi, &i_base, &dmod};
-    return launch(pl->k5, (unsigned)(np * (pl->ny / 8)), st, args, "k_c2r_z");
+    void* args[] = {&pl->dp, (void*)&pl->mapD, (void*)&phi, &i_base, &np, &dmod};
+    const long long ntile = (long long)np * (pl->ny / 8), resident = (long long)pl->n_sm * pl->k5.nl;   // persistent CTAs
+    return launch(pl->k5, (unsigned)(ntile < resident ? ntile : resident), st, args, "k_c2r_z");
 }
 static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st, double* pacc)
 {

@@ -246,23 +246,34 @@ template <class PL, int P> struct FftPass {
 // active == false take part in the barriers only.
 // `acc(pe)` returns a reference to padded slot pe = PL::pad(e) of the line (the caller chooses where
 // the slots live: a plain padded line, or a swizzled column of a TMA tile).
-template <class PL, int P, bool LAST_TO_SMEM, class Acc, class StoreLast>
-__device__ __forceinline__ void fft_tail_passes_acc(Acc acc, int tl, bool active, const cplx* __restrict__ tw, StoreLast st_last)
+// `sync()` is the barrier between the passes: __syncthreads() by default; a kernel whose lines are owned by whole
+// warps may pass a named barrier over just the warps of a line group (the passes of different lines are independent).
+struct CtaSync {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+// named barrier `id` (1..15) over `nthreads` threads (a multiple of 32: whole warps)
+struct GroupSync {
+    int id, nthreads;
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+};
+
+template <class PL, int P, bool LAST_TO_SMEM, class Acc, class StoreLast, class Sync = CtaSync>
+__device__ __forceinline__ void fft_tail_passes_acc(Acc acc, int tl, bool active, const cplx* __restrict__ tw, StoreLast st_last, Sync sync = Sync())
 {
     if constexpr (P < PL::NPASS) {
         typedef FftPass<PL, P> PS;
         typename PS::Regs rg;
-        __syncthreads(); // previous pass's writes visible
+        sync(); // previous pass's writes visible
         if (active) PS::load(rg, tl, [&](int e) { return acc(PL::pad(e)); });
         if constexpr (P == PL::NPASS - 1 && !LAST_TO_SMEM) {
             if (active) PS::compute_store(rg, tl, tw, st_last);
         } else {
-            __syncthreads(); // all reads done before the in-place writes
+            sync(); // all reads done before the in-place writes
             if (active) PS::compute_store(rg, tl, tw, [&](int e, cplx v) { acc(PL::pad(e)) = v; });
         }
-        fft_tail_passes_acc<PL, P + 1, LAST_TO_SMEM>(acc, tl, active, tw, st_last);
+        fft_tail_passes_acc<PL, P + 1, LAST_TO_SMEM>(acc, tl, active, tw, st_last, sync);
     } else {
-        if constexpr (LAST_TO_SMEM) __syncthreads();
+        if constexpr (LAST_TO_SMEM) sync();
     }
 }
 template <class PL, int P, bool LAST_TO_SMEM, class StoreLast>
