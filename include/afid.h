@@ -49,8 +49,11 @@ typedef struct afid_plan afid_plan; /* opaque; owned by the library */
  * afid_plan_create -- build a plan for an nx x ny x nz grid on the CURRENT CUDA device.
  *   nx      cells in x, 2 <= nx <= afid_max_nx()
  *   ny, nz  periodic cells; ny and nz/2 must be lengths the FFT kernels are instantiated
- *           for (afid_fft_length_supported, afid_fft_half_length_supported): powers of two
- *           times 1 or 3 (ny in 8..4096, nz/2 in 8..1024), or times 5 (ny in 40..2560, nz/2 in 40..640)
+ *           for (afid_fft_length_supported, afid_fft_half_length_supported):
+ *             ny   a multiple of 8 in 8..4096 of the form 2^a 3^b (b <= 4), or 5 2^a (40..2560);
+ *             nz/2 an even number in 8..1536 of the form 2^a 3^b (b <= 4; up to 1024 for pure powers of two
+ *                  and 1536 = 3 2^9, i.e. nz <= 3072), or 5 2^a (40..1280)
+ *           (the paper's grids, Tables 2-4: 768 x 768 x 1296, 1280 x 1024 x 256, 2048 x 3072 x 3072 slabs)
  *   xc      HOST pointer, nx+1 face coordinates (copied; caller keeps ownership)
  *   Ly, Lz  periodic box lengths (> 0)
  * The plan owns: reciprocal metrics, tridiagonal coefficients a_i, c_i, modified

@@ -87,7 +87,7 @@ __device__ __forceinline__ void pin1(double& a) { asm volatile("" : "+d"(a)); }
 // Output: B[i][jt][kz][jl] = spec_scale * X(kz), kz = 0..Nh.
 // ------------------------------------------------------------------------------------------
 template <class PL, int NL>
-__global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 384) ? 2 : 1) k_div_r2c(DevParams P, const double* __restrict__ u,
+__global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 256) ? 2 : 1) k_div_r2c(DevParams P, const double* __restrict__ u,
                                                          const double* __restrict__ v, const double* __restrict__ w,
                                                          cplx* __restrict__ B, int i_base, int np, int bmod)
 {
@@ -553,7 +553,8 @@ __host__ __device__ constexpr int k3_coef_slots(int nx, int M) { return nx + nx 
 // rows per TMA box of the K3 tile gather (box = 8 ky x 1 kz x k3_box_rows(nx) planes), and the rows the
 // boxes cover together (>= nx; the excess is out of bounds in i and arrives as zeros)
 __host__ __device__ constexpr int k3_num_boxes(int nx) { return (nx + 255) / 256; }
-__host__ __device__ constexpr int k3_box_rows(int nx) { return (nx + k3_num_boxes(nx) - 1) / k3_num_boxes(nx); }
+// (an even number of rows: a box of 64-byte rows then starts on a 128-byte boundary of the shared-memory tile, as TMA requires)
+__host__ __device__ constexpr int k3_box_rows(int nx) { return ((nx + k3_num_boxes(nx) - 1) / k3_num_boxes(nx) + 1) / 2 * 2; }
 __host__ __device__ constexpr int k3_tile_rows(int nx) { return k3_num_boxes(nx) * k3_box_rows(nx); }
 
 // KW = systems (consecutive ky) per CTA: 8 (128-byte rows), or 4 (64-byte rows; half the shared memory, so that

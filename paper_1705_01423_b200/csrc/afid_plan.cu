@@ -54,7 +54,21 @@ int fail(int code, const std::string& msg)
     X(320, 8, 8, 5, 1, 40)      \
     X(640, 16, 8, 5, 1, 40)     \
     X(1280, 16, 16, 5, 1, 80)   \
-    X(2560, 16, 16, 2, 5, 160)
+    X(2560, 16, 16, 2, 5, 160)  \
+    X(72, 12, 6, 1, 1, 6)       \
+    X(144, 12, 12, 1, 1, 12)    \
+    X(216, 6, 6, 6, 1, 36)      \
+    X(288, 12, 12, 2, 1, 24)    \
+    X(432, 12, 6, 6, 1, 36)     \
+    X(576, 12, 12, 4, 1, 48)    \
+    X(648, 12, 6, 3, 3, 54)     \
+    X(864, 12, 12, 6, 1, 72)    \
+    X(1152, 12, 12, 8, 1, 96)   \
+    X(1296, 12, 12, 3, 3, 108)  \
+    X(1728, 12, 12, 12, 1, 144) \
+    X(2304, 16, 12, 12, 1, 144) \
+    X(2592, 12, 12, 6, 3, 216)  \
+    X(3456, 12, 12, 12, 2, 288)
 
 // z-direction lines (K1, K5; complex length nz/2): plans with <= 12 elements per thread where
 // it matters, so that twice as many warps are resident while the loads are in flight
@@ -77,7 +91,26 @@ int fail(int code, const std::string& msg)
     X(80, 16, 5, 1, 1, 5)       \
     X(160, 8, 4, 5, 1, 20)      \
     X(320, 8, 8, 5, 1, 40)      \
-    X(640, 16, 8, 5, 1, 40)
+    X(640, 16, 8, 5, 1, 40)     \
+    X(1280, 16, 16, 5, 1, 80)   \
+    X(1536, 16, 16, 6, 1, 96)   \
+    X(12, 12, 1, 1, 1, 1)       \
+    X(18, 6, 3, 1, 1, 3)        \
+    X(36, 6, 6, 1, 1, 6)        \
+    X(54, 6, 3, 3, 1, 9)        \
+    X(72, 12, 6, 1, 1, 6)       \
+    X(108, 12, 3, 3, 1, 9)      \
+    X(144, 12, 12, 1, 1, 12)    \
+    X(162, 6, 3, 3, 3, 27)      \
+    X(216, 6, 6, 6, 1, 36)      \
+    X(288, 12, 12, 2, 1, 24)    \
+    X(324, 6, 6, 3, 3, 54)      \
+    X(432, 12, 6, 6, 1, 36)     \
+    X(576, 12, 12, 4, 1, 48)    \
+    X(648, 12, 6, 3, 3, 54)     \
+    X(864, 12, 12, 6, 1, 72)    \
+    X(1152, 12, 12, 8, 1, 96)   \
+    X(1296, 12, 12, 3, 3, 108)
 
 constexpr int K1_NL = 4; // lines per CTA in K1 (two CTAs fill one 128-byte row of B)
 // lines per CTA in K2 / K4: 2 (256-byte gather segments), 1 for the longest lines (two 256-thread CTAs per SM
@@ -148,7 +181,7 @@ bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5)
     }
 }
 
-constexpr int MAX_NX = 1536;
+constexpr int MAX_NX = 2048;
 
 // K3 instantiation, block size and shared memory for nx rows
 LaunchCfg select_k3(int nx, int* kw_out)
@@ -165,7 +198,8 @@ LaunchCfg select_k3(int nx, int* kw_out)
         const bool ex = (nx % 16 == 0);
         if (kw == 8) c.fn = ex ? (const void*)k_solve_x<16, true, 8, 512> : (const void*)k_solve_x<16, false, 8, 512>;
         else if (nx <= 1024) c.fn = ex ? (const void*)k_solve_x<16, true, 4, 256> : (const void*)k_solve_x<16, false, 4, 256>;
-        else c.fn = ex ? (const void*)k_solve_x<16, true, 4, 384> : (const void*)k_solve_x<16, false, 4, 384>;
+        else if (nx <= 1536) c.fn = ex ? (const void*)k_solve_x<16, true, 4, 384> : (const void*)k_solve_x<16, false, 4, 384>;
+        else c.fn = ex ? (const void*)k_solve_x<16, true, 4, 512> : (const void*)k_solve_x<16, false, 4, 512>;
     }
     const int pch = (nx + M - 1) / M;
     c.threads = kw * pch;

@@ -1,6 +1,7 @@
 """Host-side checks that need no GPU: the C-ABI library builds and loads, exports every symbol
 include/afid.h declares, fails loudly without a device, and the product never touches oracle/."""
 import ctypes
+import json
 import os
 import re
 import subprocess
@@ -50,13 +51,19 @@ def test_supported_sizes_host_queries(built_lib):
     import paper_1705_01423_b200 as afid
     for n in (16, 32, 128, 256, 512, 768, 1024, 1536, 4096, 40, 320, 1280, 2560):
         assert afid.fft_length_supported(n), n
-    for n in (0, 7, 15, 20, 100, 1000, 5000, 3200):
+    # include/afid.h: every multiple of 8 of the form 2^a 3^b in [8, 4096] with b <= 4 is a supported y length
+    for a in range(3, 13):
+        for b in range(0, 5):
+            n = 2 ** a * 3 ** b
+            if 8 <= n <= 4096:
+                assert afid.fft_length_supported(n), n
+    for n in (0, 7, 15, 20, 100, 1000, 5000, 3200, 36, 324, 1944):
         assert not afid.fft_length_supported(n), n
-    for n in (8, 768, 1024, 40, 640):
+    for n in (8, 768, 1024, 40, 640, 1280, 1536, 648, 1296, 36):
         assert afid.fft_half_length_supported(n), n
-    for n in (1280, 1536, 50):
+    for n in (2048, 50, 1728):
         assert not afid.fft_half_length_supported(n), n
-    assert afid.max_nx() >= 1024
+    assert afid.max_nx() >= 2048
 
 
 def test_no_cpu_fallback_without_device(built_lib):
@@ -96,3 +103,32 @@ def test_bench_rank_aggregation_gloo_world2():
                          capture_output=True, text=True, env=env, timeout=600)
     assert res.returncode == 0, res.stderr[-2000:]
     assert "gloo_worker ok rank 0" in res.stdout and "gloo_worker ok rank 1" in res.stdout
+
+
+def test_bench_gpus_flag_spawns_the_ranks_itself():
+    """`python bench.py --gpus 2` without a launcher starts its own two ranks (torch.distributed.run on 127.0.0.1).
+    CPU dry run through the reference arm: rank 0 alone times the oracle and prints ONE line with n_gpus = 2,
+    the other rank exits 0 without work."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference", "--workload", "C1",
+                          "--steps", "1", "--warmup", "0"], capture_output=True, text=True, env=env, timeout=600)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [ln for ln in res.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, res.stdout
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["impl"] == "reference" and line["steps"] == 1
+
+
+def test_bench_gpus_flag_fails_loudly_without_enough_devices():
+    """The CUDA arm with more ranks than visible devices exits non-zero with a clear message (no CPU fallback);
+    a launcher whose WORLD_SIZE disagrees with --gpus is an error too."""
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", str(have + 1 if have else 2)],
+                         capture_output=True, text=True, env=env, timeout=600)
+    assert res.returncode != 0
+    assert "CUDA device(s) are visible" in res.stderr, res.stderr[-500:]
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "4", "--impl", "reference"],
+                         capture_output=True, text=True, env=dict(env, WORLD_SIZE="2", RANK="0", LOCAL_RANK="0"), timeout=600)
+    assert res.returncode != 0 and "WORLD_SIZE=2" in res.stderr

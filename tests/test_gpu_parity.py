@@ -90,6 +90,43 @@ SHAPES = [
     dict(nx=3, ny=8, nz=2048, grid="uniform"),
     dict(nx=2, ny=3072, nz=16, grid="uniform"),
     dict(nx=1536, ny=8, nz=16, grid="tanh", s=3.0),
+    # every length 2^a 3^b with b >= 2 (repeated radix-3/6/12 passes), each plan at least
+    # once in y (complex length ny) and once in z (complex length nz/2)
+    dict(nx=4, ny=8, nz=24, grid="uniform"),
+    dict(nx=5, ny=16, nz=36, grid="tanh", s=3.0, Ly=0.8),
+    dict(nx=6, ny=24, nz=72, grid="tanh", s=3.0),
+    dict(nx=3, ny=48, nz=108, grid="uniform", Lz=1.7),
+    dict(nx=7, ny=72, nz=144, grid="tanh", s=3.0),
+    dict(nx=3, ny=96, nz=216, grid="tanh", s=3.0),
+    dict(nx=4, ny=144, nz=288, grid="tanh", s=3.0),
+    dict(nx=2, ny=128, nz=324, grid="uniform"),
+    dict(nx=3, ny=216, nz=432, grid="tanh", s=3.0),
+    dict(nx=2, ny=288, nz=576, grid="tanh", s=3.0),
+    dict(nx=2, ny=256, nz=648, grid="uniform"),
+    dict(nx=2, ny=432, nz=16, grid="tanh", s=3.0),
+    dict(nx=2, ny=576, nz=16, grid="tanh", s=3.0),
+    dict(nx=2, ny=648, nz=16, grid="uniform"),
+    dict(nx=2, ny=864, nz=16, grid="tanh", s=3.0),
+    dict(nx=2, ny=1152, nz=16, grid="tanh", s=3.0),
+    dict(nx=2, ny=1296, nz=16, grid="tanh", s=3.0),
+    dict(nx=2, ny=1728, nz=16, grid="uniform"),
+    dict(nx=2, ny=2304, nz=16, grid="tanh", s=3.0),
+    dict(nx=2, ny=2592, nz=16, grid="tanh", s=3.0),
+    dict(nx=2, ny=3456, nz=16, grid="uniform"),
+    dict(nx=2, ny=8, nz=864, grid="tanh", s=3.0),
+    dict(nx=2, ny=8, nz=1152, grid="tanh", s=3.0),
+    dict(nx=2, ny=8, nz=1296, grid="uniform"),
+    dict(nx=2, ny=8, nz=1728, grid="tanh", s=3.0),
+    dict(nx=2, ny=8, nz=2304, grid="tanh", s=3.0),
+    dict(nx=2, ny=8, nz=2560, grid="tanh", s=3.0),
+    dict(nx=2, ny=8, nz=2592, grid="uniform"),
+    # the paper's grid families as slabs (Table 3: 768 x 768 x 1296, wall-normal 1296;
+    # P:L319-L329 Table 2: 2048 x 3072 x 3072): nx = 1296 and 2048 = afid_max_nx(), ny = 3072, nz = 3072
+    dict(nx=1296, ny=24, nz=16, grid="tanh", s=3.0),
+    dict(nx=2048, ny=8, nz=16, grid="tanh", s=3.0),
+    dict(nx=2040, ny=8, nz=16, grid="tanh", s=3.0),
+    dict(nx=2, ny=8, nz=3072, grid="tanh", s=3.0),
+    dict(nx=3, ny=768, nz=48, grid="tanh", s=3.0),
 ]
 
 
@@ -128,7 +165,7 @@ def test_max_cfl_parity(ov):
     plan.destroy()
 
 
-@pytest.mark.parametrize("shape", [(5, 8, 16), (33, 24, 48), (64, 32, 64), (100, 16, 32), (256, 64, 64), (1030, 8, 32), (1024, 16, 64)],
+@pytest.mark.parametrize("shape", [(5, 8, 16), (33, 24, 48), (64, 32, 64), (100, 16, 32), (256, 64, 64), (1030, 8, 32), (1024, 16, 64), (2048, 8, 32), (1700, 8, 16)],
                          ids=lambda t: "x".join(map(str, t)))
 def test_xsolve_parity(shape):
     """afid_xsolve_apply against the oracle's long-double Thomas: every K3 instantiation
