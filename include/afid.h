@@ -143,6 +143,47 @@ int afid_xsolve_destroy(afid_xsolve* h);
 int afid_plan_set_pipeline(afid_plan* plan, int planes_per_batch, int rotation);
 int afid_plan_set_l2_hints(afid_plan* plan, int mask);
 
+/*
+ * afid_shard_* -- the projection sharded over `nranks` GPUs, one process per GPU.  The paper
+ * distributes the solver with pencils and SIX all-to-all transposes per projection, staged through the host
+ * (P:L103-L114); with one address space per GPU and NVLink/NVSwitch between them two
+ * exchanges are enough:
+ *   x-slabs       rank r owns the planes [xs, xe) = [nx r/R, nx (r+1)/R) for the divergence, both transforms and the
+ *                 correction (a y-z plane is local to one rank);
+ *   kz partition  rank r owns the modes kz in [ks, ke) = [nzh r/R, nzh (r+1)/R), nzh = nz/2+1, for the x-solves
+ *                 (all nx rows of a system are local to one rank);
+ *   exchange 1    forward spectrum: slabs -> kz partition;   exchange 2   solved spectrum: kz partition -> slabs;
+ *   halo          one plane of phi from the rank below (for the first u plane of the slab); the caller supplies
+ *                 the slab's upper halo plane of u (plane xe, the first plane of the rank above or the wall).
+ * The library does the arithmetic and the re-layouts; the exchanges themselves are the caller's (the Python binding
+ * uses torch.distributed all_to_all_single over NCCL, send/recv for the halo): afid_shard_layout says how many
+ * complex elements go to / come from each peer and at which offsets of the buffers afid_shard_buffers returns.
+ * One projection on rank r, all calls enqueue on `stream`:
+ *     afid_shard_forward(plan, u, v, w)          u: (xe-xs+1)*ny*nz (slab + upper halo plane), v, w: (xe-xs)*ny*nz
+ *     exchange 1   (all-to-all, counts/offsets of afid_shard_layout(..., phase 1, ...))
+ *     afid_shard_solve(plan)
+ *     exchange 2   (phase 2)
+ *     afid_shard_inverse(plan, p)                p: (xe-xs)*ny*nz <- phi of the slab
+ *     halo         p_halo <- last plane of p of rank r-1 (ny*nz doubles)
+ *     afid_shard_correct(plan, u, v, w, p, p_halo)      p_halo ignored (may be NULL) on rank 0
+ * u, v, w, p are this rank's slabs (DEVICE, same layout as afid_project); the slab's own planes of u, v, w are
+ * updated in place (the halo plane of u is read only).  The result equals afid_project on the whole grid bit for
+ * bit: the same kernels run on the same lines and systems.  afid_max_cfl on a sharded plan returns the slab's
+ * maximum (the caller all-reduces it).  afid_project, the stage taps, afid_xsolve_* and the accumulate
+ * mode need an unsharded plan.  nranks <= 64, nranks <= nx, nranks <= nz/2+1.
+ * afid_shard_bounds / afid_shard_layout are host arithmetic only (usable without a device).
+ */
+afid_plan* afid_shard_plan_create(int nx, int ny, int nz, const double* xc, double Ly, double Lz, int rank, int nranks);
+int afid_shard_bounds(int n, int nranks, int rank, int* lo, int* hi);   /* part `rank` of n items: [n rank/nranks, n (rank+1)/nranks) */
+int afid_shard_layout(int nx, int ny, int nz, int nranks, int rank, int phase, long long* send_count, long long* send_off,
+                      long long* recv_count, long long* recv_off);       /* HOST arrays of nranks entries each */
+int afid_shard_buffers(afid_plan* plan, int phase, void** send, void** recv);
+int afid_shard_info(const afid_plan* plan, int* rank, int* nranks, int* xs, int* xe, int* ks, int* ke);
+int afid_shard_forward(afid_plan* plan, const double* u, const double* v, const double* w, void* stream);
+int afid_shard_solve(afid_plan* plan, void* stream);
+int afid_shard_inverse(afid_plan* plan, double* p, void* stream);
+int afid_shard_correct(afid_plan* plan, double* u, double* v, double* w, double* p, const double* p_halo, void* stream);
+
 /* afid_plan_destroy -- free the plan's device and host memory.  NULL is a no-op.
  * The caller must have synchronised any stream still using the plan. */
 int afid_plan_destroy(afid_plan* plan);

@@ -24,7 +24,9 @@ SYMBOLS = ["afid_plan_create", "afid_project", "afid_plan_destroy", "afid_plan_w
            "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version",
            "afid_plan_enable_timing", "afid_plan_kernel_times", "afid_plan_kernel_name",
            "afid_fft_half_length_supported", "afid_max_cfl", "afid_plan_set_accumulate", "afid_xsolve_create", "afid_xsolve_apply",
-           "afid_xsolve_destroy", "afid_plan_set_pipeline", "afid_plan_set_l2_hints", "afid_plan_num_timed"]
+           "afid_xsolve_destroy", "afid_plan_set_pipeline", "afid_plan_set_l2_hints", "afid_plan_num_timed",
+           "afid_shard_plan_create", "afid_shard_bounds", "afid_shard_layout", "afid_shard_buffers", "afid_shard_info",
+           "afid_shard_forward", "afid_shard_solve", "afid_shard_inverse", "afid_shard_correct"]
 
 _lib = None
 
@@ -88,6 +90,24 @@ def lib():
         L.afid_plan_num_timed.argtypes = [vp]
         L.afid_plan_kernel_name.restype = C.c_char_p
         L.afid_plan_kernel_name.argtypes = [vp, i]
+        L.afid_shard_plan_create.restype = vp
+        L.afid_shard_plan_create.argtypes = [i, i, i, vp, d, d, i, i]
+        L.afid_shard_bounds.restype = i
+        L.afid_shard_bounds.argtypes = [i, i, i, vp, vp]
+        L.afid_shard_layout.restype = i
+        L.afid_shard_layout.argtypes = [i, i, i, i, i, i, vp, vp, vp, vp]
+        L.afid_shard_buffers.restype = i
+        L.afid_shard_buffers.argtypes = [vp, i, vp, vp]
+        L.afid_shard_info.restype = i
+        L.afid_shard_info.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        L.afid_shard_forward.restype = i
+        L.afid_shard_forward.argtypes = [vp, vp, vp, vp, vp]
+        L.afid_shard_solve.restype = i
+        L.afid_shard_solve.argtypes = [vp, vp]
+        L.afid_shard_inverse.restype = i
+        L.afid_shard_inverse.argtypes = [vp, vp, vp]
+        L.afid_shard_correct.restype = i
+        L.afid_shard_correct.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -245,6 +265,123 @@ class XSolve:
     def destroy(self):
         if getattr(self, "_h", None):
             lib().afid_xsolve_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+# ------------------------------------------------------------------------------------------
+# the projection sharded over ranks (include/afid.h, afid_shard_*)
+# ------------------------------------------------------------------------------------------
+def shard_bounds(n, nranks, rank):
+    """afid_shard_bounds: part `rank` of n items, [lo, hi) (host arithmetic, no device)."""
+    lo, hi = C.c_int(0), C.c_int(0)
+    _check(lib().afid_shard_bounds(int(n), int(nranks), int(rank), C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
+
+
+def shard_layout(nx, ny, nz, nranks, rank, phase):
+    """afid_shard_layout: (send_count, send_off, recv_count, recv_off), lists of nranks ints in complex elements
+    (host arithmetic, no device)."""
+    arr = [(C.c_longlong * nranks)() for _ in range(4)]
+    _check(lib().afid_shard_layout(int(nx), int(ny), int(nz), int(nranks), int(rank), int(phase),
+                                   *[C.cast(a, C.c_void_p) for a in arr]))
+    return tuple([int(x) for x in a] for a in arr)
+
+
+class _DevView:
+    """A raw device allocation as a __cuda_array_interface__ object (so torch can wrap it without a copy)."""
+
+    def __init__(self, ptr, nbytes):
+        self.__cuda_array_interface__ = {"shape": (nbytes // 8,), "typestr": "<f8", "data": (int(ptr), False), "version": 3}
+
+
+class ShardPlan:
+    """afid_shard_plan_create and the four stages of a sharded projection for rank `rank` of `nranks`.
+    nx is the GLOBAL number of planes, xc the global nx+1 faces; u holds this rank's planes xs..xe (the slab plus
+    its upper halo plane), v, w, p the planes xs..xe-1."""
+
+    def __init__(self, nx, ny, nz, xc, Ly, Lz, rank, nranks):
+        import numpy as np
+        xc = np.ascontiguousarray(xc, dtype=np.float64)
+        if xc.size != nx + 1:
+            raise ValueError("xc must hold nx+1 face coordinates")
+        self.gnx, self.ny, self.nz, self.rank, self.nranks = int(nx), int(ny), int(nz), int(rank), int(nranks)
+        self.nzh = self.nz // 2 + 1
+        self._h = lib().afid_shard_plan_create(self.gnx, self.ny, self.nz, xc.ctypes.data_as(C.c_void_p), float(Ly), float(Lz),
+                                               self.rank, self.nranks)
+        if not self._h:
+            raise AfidError(*_last_error())
+        v = [C.c_int(0) for _ in range(6)]
+        _check(lib().afid_shard_info(self._h, *[C.byref(x) for x in v]))
+        _, _, self.xs, self.xe, self.ks, self.ke = [x.value for x in v]
+        self.nxl, self.nkz = self.xe - self.xs, self.ke - self.ks
+        self.layout = {ph: shard_layout(self.gnx, self.ny, self.nz, self.nranks, self.rank, ph) for ph in (1, 2)}
+
+    _stream = Plan._stream
+
+    def buffers(self, phase):
+        """afid_shard_buffers: (send, recv) as flat complex128 CUDA tensors over the plan's work arrays."""
+        import torch
+        s, r = C.c_void_p(0), C.c_void_p(0)
+        _check(lib().afid_shard_buffers(self._h, int(phase), C.byref(s), C.byref(r)))
+        n = max(self.nxl * self.nzh, self.gnx * self.nkz) * self.ny * 16
+        dev = torch.device("cuda", torch.cuda.current_device())
+        return tuple(torch.view_as_complex(torch.as_tensor(_DevView(x.value, n), device=dev).view(-1, 2)) for x in (s, r))
+
+    def forward(self, u, v, w, stream=None):
+        n = self.nxl * self.ny * self.nz
+        _check(lib().afid_shard_forward(self._h, _dev_ptr(u, n + self.ny * self.nz, "u"), _dev_ptr(v, n, "v"), _dev_ptr(w, n, "w"),
+                                        self._stream(stream)))
+
+    def solve(self, stream=None):
+        _check(lib().afid_shard_solve(self._h, self._stream(stream)))
+
+    def inverse(self, p, stream=None):
+        _check(lib().afid_shard_inverse(self._h, _dev_ptr(p, self.nxl * self.ny * self.nz, "p"), self._stream(stream)))
+
+    def correct(self, u, v, w, p, p_halo, stream=None):
+        n = self.nxl * self.ny * self.nz
+        ph = C.c_void_p(0) if p_halo is None else _dev_ptr(p_halo, self.ny * self.nz, "p_halo")
+        _check(lib().afid_shard_correct(self._h, _dev_ptr(u, n + self.ny * self.nz, "u"), _dev_ptr(v, n, "v"), _dev_ptr(w, n, "w"),
+                                        _dev_ptr(p, n, "p"), ph, self._stream(stream)))
+
+    def exchange(self, phase, group=None):
+        """The all-to-all of `phase` over torch.distributed (NCCL): plumbing only, the blocks are already laid out."""
+        import torch.distributed as dist
+        sc, so, rc, ro = self.layout[phase]
+        send, recv = self.buffers(phase)
+        # the per-peer blocks are back to back in rank order, so the split sizes describe them completely
+        dist.all_to_all_single(recv[:sum(rc)], send[:sum(sc)], output_split_sizes=rc, input_split_sizes=sc, group=group)
+
+    def project(self, u, v, w, p, group=None):
+        """One sharded projection on this rank (all ranks of `group` call it): stages, two exchanges, phi halo."""
+        import torch
+        import torch.distributed as dist
+        self.forward(u, v, w)
+        self.exchange(1, group)
+        self.solve()
+        self.exchange(2, group)
+        self.inverse(p)
+        halo = None
+        ops = []
+        if self.rank + 1 < self.nranks:
+            ops.append(dist.P2POp(dist.isend, p[self.nxl - 1].contiguous(), self.rank + 1, group))
+        if self.rank > 0:
+            halo = torch.empty((self.ny, self.nz), dtype=torch.float64, device=p.device)
+            ops.append(dist.P2POp(dist.irecv, halo, self.rank - 1, group))
+        if ops:
+            for req in dist.batch_isend_irecv(ops):
+                req.wait()
+        self.correct(u, v, w, p, halo)
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().afid_plan_destroy(self._h)
             self._h = None
 
     def __del__(self):

@@ -38,6 +38,7 @@ struct DevParams {
     const cplx* tw_z;           // [nz/2+1] exp(-2 pi i k/nz)
     double inv_vol;             // 1/sum dx_i
     int hints;                  // L2 eviction-priority switches (bit mask, see l2_policy users)
+    int has_mean;               // K3: this launch holds the mean mode (ky, kz) = (0, 0) as its first system (sharded plans: only the rank owning kz = 0)
 };
 
 // L2 eviction priorities (PTX createpolicy): 0 = normal, 1 = evict_first (streamed once), 2 = evict_last (kept)
@@ -427,9 +428,11 @@ __global__ void __launch_bounds__(LPR* PL::TPL, 1) k_c2r_z(DevParams P, const __
 constexpr int K6_JL = 4, K6_TX = 64, K6_U = 4;
 
 __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const double* __restrict__ p, double* __restrict__ u,
-                                                          double* __restrict__ v, double* __restrict__ w, int i_base, int np, double* __restrict__ pacc)
+                                                          double* __restrict__ v, double* __restrict__ w, int i_base, int np, double* __restrict__ pacc,
+                                                          const double* __restrict__ p_halo)
 {
-    // `p` holds phi; if pacc != nullptr the pressure is accumulated as well: pacc += phi (P:L91, P:L116 delta form)
+    // `p` holds phi; if pacc != nullptr the pressure is accumulated as well: pacc += phi (P:L91, P:L116 delta form).
+    // p_halo (sharded plans): the plane of phi below this slab's first plane (nullptr: plane 0 is the wall)
     constexpr int JL = K6_JL, TX = K6_TX, U = K6_U;
     // this launch covers planes i_base .. i_base+np-1.
     // CTA order: j-chunks of 32 lines outermost, then i, then the group inside the chunk, so that
@@ -450,10 +453,10 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const dou
     const size_t ol = ((size_t)i * P.ny + j) * P.nz;
     const double* pl = p + ol;
     const double* pjm = p + ((size_t)i * P.ny + jm) * P.nz;
-    const double* pim = pl - plane;          // only dereferenced for i >= 1
+    const double* pim = (i >= 1) ? pl - plane : p_halo + (size_t)j * P.nz;   // only dereferenced if has_u
     double *ul = u + ol, *vl = v + ol, *wl = w + ol;
     const int nzh2 = P.nz / 2;
-    const bool has_u = (i >= 1);
+    const bool has_u = (i >= 1) || (p_halo != nullptr);
     const double rdc = has_u ? __ldg(&P.rdc[i]) : 0.0, rdy = P.rdy, rdz = P.rdz;
     const unsigned long long pol_in = l2_policy((P.hints & 1) ? 1 : 0), pol_out = l2_policy((P.hints & 8) ? 1 : 0);
     for (int k0 = threadIdx.x; k0 < nzh2; k0 += TX * U) {
@@ -592,7 +595,7 @@ __global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_consta
     mbar_wait(&bar, 0);
     auto ld_ac = [&](int i) -> double2 { return coef[i + i / M]; };   // {a_i, c_i}: one conflict-free LDS.128
     const double lam = __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]);
-    const bool cta_singular = (blockIdx.x == 0);
+    const bool cta_singular = (blockIdx.x == 0) && P.has_mean;
     const int i0 = q * M;
     const int i1 = min(i0 + M, nx) - 1; // interface row of this chunk
     double* bA = red;

@@ -248,10 +248,17 @@ bool make_map3(CUtensorMap* m, void* base, uint64_t d0, uint64_t d1, uint64_t d2
 constexpr int PIPE_STREAMS = 3;
 constexpr int PIPE_EVENTS = 8;   // per kind; >= the largest rotation depth + 1
 
+constexpr int MAX_RANKS = 64;   // sharded plans
+
 struct afid_plan {
-    int nx, ny, nz, nzh;
+    int nx, ny, nz, nzh;   // nx = planes of THIS plan's x-slab (= the whole grid for an unsharded plan)
     int device;        // the device the plan was created on (its work arrays and tensor maps live there)
-    DevParams dp;
+    // sharded plans: the global grid has gnx planes; this rank owns the x-slab [bx[rank], bx[rank+1]) for the
+    // divergence, the transforms and the correction, and the modes kz in [bk[rank], bk[rank+1]) for the x-solves
+    int gnx, rank, nranks;
+    int bx[MAX_RANKS + 1], bk[MAX_RANKS + 1];
+    DevParams dp;      // slab kernels (K1, K2, K4, K5, K6): nx = slab planes, metric tables offset to the slab
+    DevParams dps;     // x-solve (K3): nx = gnx, nzh = this rank's kz count, lamz offset to its first kz
     void* tables;      // one device allocation holding all tables
     size_t tables_bytes;
     cplx* ws[2];       // work arrays, nx*nzh*ny complex each
@@ -339,7 +346,13 @@ static void discard_plan(afid_plan* pl)
 
 extern "C" {
 
-AFID_EXPORT afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly, double Lz)
+} // extern "C"
+
+// balanced contiguous partition of n items over R parts: part r = [n r / R, n (r+1) / R)
+static int part_bound(int n, int R, int r) { return (int)((long long)n * r / R); }
+
+// nx = GLOBAL number of planes; the plan built is rank `rank` of `nranks` (1 rank: the whole problem)
+static afid_plan* create_impl(int nx, int ny, int nz, const double* xc, double Ly, double Lz, int rank, int nranks)
 {
     g_err.clear();
     g_err_code = 0;
@@ -350,12 +363,17 @@ AFID_EXPORT afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc
     for (int i = 0; i <= nx; ++i)
         if (!std::isfinite(xc[i]) || (i > 0 && !(xc[i] > xc[i - 1]))) { fail(AFID_ERR_GRID, "xc must be finite and strictly increasing"); return nullptr; }
     const int nh = nz / 2;
+    if (nranks < 1 || nranks > MAX_RANKS || rank < 0 || rank >= nranks) { fail(AFID_ERR_UNSUPPORTED_SIZE, "rank / nranks out of range (nranks <= 64)"); return nullptr; }
+    if (nranks > nx || nranks > nh + 1) { fail(AFID_ERR_UNSUPPORTED_SIZE, "more ranks than x-planes or kz modes"); return nullptr; }
     afid_plan* pl = new (std::nothrow) afid_plan();
     if (!pl) { fail(AFID_ERR_NOMEM, "host allocation failed"); return nullptr; }
     std::memset(pl, 0, sizeof(*pl));
     if (!lookup_fft_y(ny, &pl->k2, &pl->k4)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "ny is not a supported FFT length"); return nullptr; }
     if (!lookup_fft_z(nh, &pl->k1, &pl->k5)) { delete pl; fail(AFID_ERR_UNSUPPORTED_SIZE, "nz/2 is not a supported FFT length"); return nullptr; }
-    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
+    pl->gnx = nx; pl->rank = rank; pl->nranks = nranks;
+    for (int r = 0; r <= nranks; ++r) { pl->bx[r] = part_bound(nx, nranks, r); pl->bk[r] = part_bound(nh + 1, nranks, r); }
+    const int xs = pl->bx[rank], nxl = pl->bx[rank + 1] - xs, ks = pl->bk[rank], nkz = pl->bk[rank + 1] - ks;
+    pl->nx = nxl; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
 
     // ---- K3 configuration
     pl->k3 = select_k3(nx, &pl->k3_kw);
@@ -426,18 +444,21 @@ AFID_EXPORT afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc
         if (cudaMemcpy((char*)pl->tables + it.off, it.src, it.bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
             discard_plan(pl); fail(AFID_ERR_CUDA, "cudaMemcpy(tables) failed"); return nullptr;
         }
-    pl->ws_bytes = (size_t)nx * pl->nzh * ny * sizeof(cplx);
+    {   // a work array holds the slab's half spectrum (nxl planes x all kz) or this rank's modes (all planes x nkz)
+        const size_t a = (size_t)nxl * pl->nzh, b = (size_t)nx * nkz;
+        pl->ws_bytes = (a > b ? a : b) * ny * sizeof(cplx);
+    }
     for (int b = 0; b < 2; ++b)
         if (cudaMalloc((void**)&pl->ws[b], pl->ws_bytes) != cudaSuccess) {
             cudaGetLastError();
             discard_plan(pl); fail(AFID_ERR_NOMEM, "cudaMalloc(work arrays) failed"); return nullptr;
         }
-    if (!make_map3(&pl->mapC, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)nx, (uint64_t)pl->nzh, 2 * (uint32_t)pl->k3_kw, (uint32_t)k3_box_rows(nx), 1,
+    if (!make_map3(&pl->mapC, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)nx, (uint64_t)nkz, 2 * (uint32_t)pl->k3_kw, (uint32_t)k3_box_rows(nx), 1,
                    CU_TENSOR_MAP_SWIZZLE_NONE)) {
         discard_plan(pl);
         fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed"); return nullptr;
     }
-    if (!make_map3(&pl->mapD, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)pl->nzh, (uint64_t)nx, 16, (uint32_t)k5_box_rows(nh), 1,
+    if (!make_map3(&pl->mapD, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)pl->nzh, (uint64_t)nxl, 16, (uint32_t)k5_box_rows(nh), 1,
                    CU_TENSOR_MAP_SWIZZLE_128B)) {
         discard_plan(pl);
         fail(AFID_ERR_CUDA, "cuTensorMapEncodeTiled failed"); return nullptr;
@@ -460,7 +481,22 @@ AFID_EXPORT afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc
     d.tw_z = (const cplx*)(tb + items[9].off);
     d.inv_vol = (double)(1.0L / vol);
     d.hints = 0;
+    d.has_mean = (ks == 0) ? 1 : 0;
+    pl->dps = d;                 // x-solve: all planes, this rank's kz
+    pl->dps.nzh = nkz;
+    pl->dps.lamz = d.lamz + ks;
+    d.nx = nxl;                  // slab kernels: this rank's planes, all kz
+    d.rdx += xs;
+    d.rdc += xs;
+    d.dxw += xs;
     return pl;
+}
+
+extern "C" {
+
+AFID_EXPORT afid_plan* afid_plan_create(int nx, int ny, int nz, const double* xc, double Ly, double Lz)
+{
+    return create_impl(nx, ny, nz, xc, Ly, Lz, 0, 1);
 }
 
 AFID_EXPORT int afid_plan_destroy(afid_plan* pl)
@@ -571,9 +607,10 @@ static int launch_k5(afid_plan* pl, double* phi, int i_base, int np, int dmod, c
     const long long ntile = (long long)np * (pl->ny / 8), resident = (long long)pl->n_sm * pl->k5.nl;   // persistent CTAs
     return launch(pl->k5, (unsigned)(ntile < resident ? ntile : resident), st, args, "k_c2r_z");
 }
-static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st, double* pacc)
+static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double* p, int i_base, int np, cudaStream_t st, double* pacc,
+                          const double* p_halo = nullptr)
 {
-    void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, &i_base, &np, (void*)&pacc};
+    void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, &i_base, &np, (void*)&pacc, (void*)&p_halo};
     cudaError_t e = cudaLaunchKernel((const void*)k_correct, dim3((unsigned)(np * (pl->ny / K6_JL))), dim3(K6_TX, K6_JL), args, 0, st);
     if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_correct: ") + cudaGetErrorString(e));
     return AFID_OK;
@@ -625,8 +662,8 @@ static int run_forward(afid_plan* pl, const double* u, const double* v, const do
 // K3: C (always ws[1]: the tensor map is bound to it) -> T
 static int run_solve(afid_plan* pl, cplx* outT, cudaStream_t st)
 {
-    void* args[] = {&pl->dp, (void*)&pl->mapC, (void*)&outT};
-    return launch(pl->k3, (unsigned)(pl->nzh * (pl->ny / pl->k3_kw)), st, args, "k_solve_x");
+    void* args[] = {&pl->dps, (void*)&pl->mapC, (void*)&outT};
+    return launch(pl->k3, (unsigned)(pl->dps.nzh * (pl->ny / pl->k3_kw)), st, args, "k_solve_x");
 }
 
 // K4 + K5 + K6: T -> D -> p, u, v, w
@@ -670,6 +707,7 @@ AFID_EXPORT int afid_project(afid_plan* pl, double* u, double* v, double* w, dou
     int rc;
     if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(p, "p"))) return rc;
     if ((rc = check_device(pl))) return rc;
+    if (pl->nranks != 1) return fail(AFID_ERR_UNSUPPORTED_SIZE, "afid_project on a sharded plan: use the afid_shard_* stages");
     cudaStream_t st = (cudaStream_t)stream;
     const bool tm = pl->timing;
     cplx* wsB = pl->ws[0];
@@ -685,6 +723,138 @@ AFID_EXPORT int afid_project(afid_plan* pl, double* u, double* v, double* w, dou
         pl->ev_valid = true;
     }
     return AFID_OK;
+}
+
+// ---- the projection sharded over ranks (one process per GPU) -----------------------------------
+// Two exchanges per projection instead of the paper's six all-to-alls: x-slabs for the
+// divergence, both transforms and the correction, a kz partition for the x-solves.  C and T are kz-major, so the
+// blocks that travel are contiguous on the sending side of exchange 1 and on the receiving side of exchange 2;
+// the other two sides are one strided device copy per peer (the re-layouts below).
+AFID_EXPORT afid_plan* afid_shard_plan_create(int nx, int ny, int nz, const double* xc, double Ly, double Lz, int rank, int nranks)
+{
+    return create_impl(nx, ny, nz, xc, Ly, Lz, rank, nranks);
+}
+
+AFID_EXPORT int afid_shard_bounds(int n, int nranks, int rank, int* lo, int* hi)
+{
+    if (nranks < 1 || rank < 0 || rank >= nranks || n < nranks || !lo || !hi) return fail(AFID_ERR_UNSUPPORTED_SIZE, "afid_shard_bounds: bad arguments");
+    *lo = part_bound(n, nranks, rank);
+    *hi = part_bound(n, nranks, rank + 1);
+    return AFID_OK;
+}
+
+// Host arithmetic only (no device, no plan): what rank `rank` sends to / receives from every peer in exchange
+// `phase` (1: forward spectrum C, slabs -> kz partition; 2: solved spectrum T, kz partition -> slabs), in complex
+// elements (16 bytes), as offsets into the send / receive buffers of afid_shard_buffers.
+AFID_EXPORT int afid_shard_layout(int nx, int ny, int nz, int nranks, int rank, int phase, long long* send_count, long long* send_off,
+                                  long long* recv_count, long long* recv_off)
+{
+    if (nranks < 1 || nranks > MAX_RANKS || rank < 0 || rank >= nranks || nx < nranks || nz / 2 + 1 < nranks || (phase != 1 && phase != 2) ||
+        !send_count || !send_off || !recv_count || !recv_off)
+        return fail(AFID_ERR_UNSUPPORTED_SIZE, "afid_shard_layout: bad arguments");
+    const int nzh = nz / 2 + 1;
+    auto bx = [&](int r) { return (long long)part_bound(nx, nranks, r); };
+    auto bk = [&](int r) { return (long long)part_bound(nzh, nranks, r); };
+    const long long nxl = bx(rank + 1) - bx(rank), nkz = bk(rank + 1) - bk(rank);
+    for (int r = 0; r < nranks; ++r) {
+        const long long nxr = bx(r + 1) - bx(r), nkr = bk(r + 1) - bk(r);
+        if (phase == 1) {   // send C_loc[kz of r][my planes][ky]; receive [my kz][planes of r][ky]
+            send_count[r] = nkr * nxl * ny;  send_off[r] = bk(r) * nxl * ny;
+            recv_count[r] = nkz * nxr * ny;  recv_off[r] = nkz * bx(r) * ny;
+        } else {            // send [my kz][kyt][planes of r][8]; receive T_loc[kz of r][kyt][my planes][8]
+            send_count[r] = nkz * nxr * ny;  send_off[r] = nkz * bx(r) * ny;
+            recv_count[r] = nkr * nxl * ny;  recv_off[r] = bk(r) * nxl * ny;
+        }
+    }
+    return AFID_OK;
+}
+
+// device pointers of the buffers exchange `phase` sends from / receives into (both are the plan's work arrays)
+AFID_EXPORT int afid_shard_buffers(afid_plan* pl, int phase, void** send, void** recv)
+{
+    if (!pl || !send || !recv) return fail(AFID_ERR_NULL, "plan, send or recv is NULL");
+    if (phase != 1 && phase != 2) return fail(AFID_ERR_UNSUPPORTED_SIZE, "phase must be 1 or 2");
+    *send = pl->ws[1];
+    *recv = pl->ws[0];
+    return AFID_OK;
+}
+
+AFID_EXPORT int afid_shard_info(const afid_plan* pl, int* rank, int* nranks, int* xs, int* xe, int* ks, int* ke)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    if (rank) *rank = pl->rank;
+    if (nranks) *nranks = pl->nranks;
+    if (xs) *xs = pl->bx[pl->rank];
+    if (xe) *xe = pl->bx[pl->rank + 1];
+    if (ks) *ks = pl->bk[pl->rank];
+    if (ke) *ke = pl->bk[pl->rank + 1];
+    return AFID_OK;
+}
+
+// stage 1: divergence + forward transforms of this rank's slab; the send buffer of exchange 1 is ready afterwards
+AFID_EXPORT int afid_shard_forward(afid_plan* pl, const double* u, const double* v, const double* w, void* stream)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    int rc;
+    if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w"))) return rc;
+    if ((rc = check_device(pl))) return rc;
+    return run_forward(pl, u, v, w, pl->ws[0], pl->ws[1], (cudaStream_t)stream, nullptr);
+}
+
+static int copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t width, size_t height, cudaStream_t st)
+{
+    cudaError_t e = cudaMemcpy2DAsync(dst, dpitch, src, spitch, width, height, cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaMemcpy2DAsync: ") + cudaGetErrorString(e));
+    return AFID_OK;
+}
+
+// stage 2 (after exchange 1): received blocks -> C[kz][i][ky] over all planes, x-solves, T -> per-peer send blocks
+AFID_EXPORT int afid_shard_solve(afid_plan* pl, void* stream)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    int rc;
+    if ((rc = check_device(pl))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t ny = pl->ny, gnx = pl->gnx, nkz = pl->dps.nzh, E = sizeof(cplx);
+    {   // block of peer r: [nkz][planes of r][ny] -> rows bx[r].. of every kz  (one rank: a plain copy, the exchange still runs)
+        for (int r = 0; r < pl->nranks; ++r) {
+            const size_t x0 = pl->bx[r], nxr = pl->bx[r + 1] - pl->bx[r];
+            if ((rc = copy2d(pl->ws[1] + x0 * ny, gnx * ny * E, pl->ws[0] + nkz * x0 * ny, nxr * ny * E, nxr * ny * E, nkz, st))) return rc;
+        }
+    }
+    if ((rc = run_solve(pl, pl->ws[0], st))) return rc;
+    {   // T[kz][kyt][i][8] -> block of peer r: [nkz][kyt][planes of r][8]
+        const size_t rows = nkz * (ny / 8);
+        for (int r = 0; r < pl->nranks; ++r) {
+            const size_t x0 = pl->bx[r], nxr = pl->bx[r + 1] - pl->bx[r];
+            if ((rc = copy2d(pl->ws[1] + nkz * x0 * ny, nxr * 8 * E, pl->ws[0] + x0 * 8, gnx * 8 * E, nxr * 8 * E, rows, st))) return rc;
+        }
+    }
+    return AFID_OK;
+}
+
+// stage 3 (after exchange 2): inverse transforms of this rank's slab, phi -> p
+AFID_EXPORT int afid_shard_inverse(afid_plan* pl, double* p, void* stream)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    int rc;
+    if ((rc = check_ptr(p, "p"))) return rc;
+    if ((rc = check_device(pl))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if ((rc = launch_k4(pl, pl->ws[0], pl->ws[1], 0, pl->nx, pl->nx, st))) return rc;
+    return launch_k5(pl, p, 0, pl->nx, pl->nx, st);
+}
+
+// stage 4 (after the halo exchange of phi): correction of this rank's slab.  p_halo = the last plane of phi of the
+// rank below (ny*nz doubles, device), NULL on rank 0 (plane 0 is the wall).
+AFID_EXPORT int afid_shard_correct(afid_plan* pl, double* u, double* v, double* w, double* p, const double* p_halo, void* stream)
+{
+    if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
+    int rc;
+    if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(p, "p"))) return rc;
+    if (pl->rank > 0 && (rc = check_ptr(p_halo, "p_halo"))) return rc;
+    if ((rc = check_device(pl))) return rc;
+    return launch_correct(pl, u, v, w, p, 0, pl->nx, (cudaStream_t)stream, nullptr, pl->rank > 0 ? p_halo : nullptr);
 }
 
 AFID_EXPORT int afid_max_cfl(afid_plan* pl, const double* u, const double* v, const double* w, double* cfl, void* stream)
@@ -726,6 +896,7 @@ AFID_EXPORT afid_xsolve* afid_xsolve_create(afid_plan* pl, const double* a_in, c
     g_err.clear();
     g_err_code = 0;
     if (!pl || !a_in || !c_in || !lam) { fail(AFID_ERR_NULL, "plan, a, c or lam is NULL"); return nullptr; }
+    if (pl->nranks != 1) { fail(AFID_ERR_UNSUPPORTED_SIZE, "afid_xsolve_create needs an unsharded plan (the columns span all x)"); return nullptr; }
     const int nx = pl->nx;
     for (int i = 0; i < nx; ++i)
         if (!(a_in[i] >= 0.0) || !(c_in[i] >= 0.0) || !(lam[i] > 0.0) || !std::isfinite(a_in[i]) || !std::isfinite(c_in[i]) || !std::isfinite(lam[i])) {
@@ -923,6 +1094,7 @@ AFID_EXPORT int afid_stage_forward(afid_plan* pl, const double* u, const double*
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     int rc;
     if ((rc = check_ptr(u, "u")) || (rc = check_ptr(v, "v")) || (rc = check_ptr(w, "w")) || (rc = check_ptr(spec, "spec"))) return rc;
+    if (pl->nranks != 1) return fail(AFID_ERR_UNSUPPORTED_SIZE, "stage taps need an unsharded plan");
     cudaStream_t st = (cudaStream_t)stream;
     if ((rc = run_forward(pl, u, v, w, pl->ws[0], pl->ws[1], st, nullptr))) return rc;
     k_tap_C_to_api<<<pl->n_sm * 8, 256, 0, st>>>(pl->dp, pl->ws[1], (cplx*)spec, 1);
@@ -936,6 +1108,7 @@ AFID_EXPORT int afid_stage_solve(afid_plan* pl, double* spec, void* stream)
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     int rc;
     if ((rc = check_ptr(spec, "spec"))) return rc;
+    if (pl->nranks != 1) return fail(AFID_ERR_UNSUPPORTED_SIZE, "stage taps need an unsharded plan");
     cudaStream_t st = (cudaStream_t)stream;
     k_tap_C_to_api<<<pl->n_sm * 8, 256, 0, st>>>(pl->dp, pl->ws[1], (cplx*)spec, 0);
     if ((rc = run_solve(pl, pl->ws[0], st))) return rc;

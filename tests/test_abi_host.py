@@ -132,3 +132,31 @@ def test_bench_gpus_flag_fails_loudly_without_enough_devices():
     res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "4", "--impl", "reference"],
                          capture_output=True, text=True, env=dict(env, WORLD_SIZE="2", RANK="0", LOCAL_RANK="0"), timeout=600)
     assert res.returncode != 0 and "WORLD_SIZE=2" in res.stderr
+
+
+@pytest.mark.parametrize("world,shape", [(2, (20, 24, 48)), (3, (13, 8, 16)), (4, (65, 32, 64))])
+def test_shard_exchange_schedule_gloo(world, shape):
+    """the two all-to-alls of the sharded projection, world_size > 1 on CPU over gloo, with the
+    counts / offsets of afid_shard_layout (host arithmetic of the library, no device)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    res = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={world}",
+                          "--master-addr", "127.0.0.1", "--master-port", str(port),
+                          os.path.join(ROOT, "tests", "gloo_shard_worker.py")] + [str(x) for x in shape],
+                         capture_output=True, text=True, env=env, timeout=600)
+    assert res.returncode == 0, res.stdout[-1500:] + res.stderr[-3000:]
+    assert res.stdout.count("gloo_shard_worker ok") == world
+
+
+def test_shard_bounds_partition():
+    import paper_1705_01423_b200 as afid
+    for n, R in ((1024, 8), (769, 8), (13, 3), (5, 5)):
+        b = [afid.shard_bounds(n, R, r) for r in range(R)]
+        assert b[0][0] == 0 and b[-1][1] == n
+        assert all(b[r][1] == b[r + 1][0] for r in range(R - 1)) and all(hi > lo for lo, hi in b)
+        assert max(hi - lo for lo, hi in b) - min(hi - lo for lo, hi in b) <= 1
+    with pytest.raises(afid.AfidError):
+        afid.shard_bounds(3, 4, 0)
