@@ -31,6 +31,7 @@ struct DevParams {
     const double* dxw;          // [nx]   dx_i (weights of the mean)
     const double* ca;           // [nx]   a_i = 1/(dx_i dc_i),   a_0 = 0
     const double* cc;           // [nx]   c_i = 1/(dx_i dc_{i+1}), c_{nx-1} = 0
+    const double2* acp;         // K3: {a_i, c_i} in the kernel's shared-memory layout (chunk q at [q (M+1), q (M+1) + M]), k3_coef_slots entries
     const double* lamy;         // [ny]   modified wavenumbers in y
     const double* lamz;         // [nzh]  modified wavenumbers in z
     const cplx* tw_y;           // [ny]    exp(-2 pi i k/ny)
@@ -38,6 +39,7 @@ struct DevParams {
     const cplx* tw_z;           // [nz/2+1] exp(-2 pi i k/nz)
     double inv_vol;             // 1/sum dx_i
     int hints;                  // L2 eviction-priority switches (bit mask, see l2_policy users)
+    int k3_prefetch;            // K3: a CTA prefetches the tile of CTA blockIdx.x + k3_prefetch into L2 (0 = off)
     int has_mean;               // K3: this launch holds the mean mode (ky, kz) = (0, 0) as its first system (sharded plans: only the rank owning kz = 0)
 };
 
@@ -530,7 +532,8 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const dou
 // 1/x for a positive, normal x, to fp64 round-off.  The 64-bit MUFU (rcp.approx.f64, MUFU.RCP64H) is
 // what the x-solve was bound by on B200 (XU pipe at 160 % of its sustained peak in ncu), so the seed is a
 // 32-bit MUFU.RCP of the mantissa, moved between the formats with integer operations only (no F2F
-// conversions: they use the same slow pipe), followed by two Newton steps (2^-22 -> 2^-44 -> 2^-88).
+// conversions: they use the same slow pipe), followed by ONE third-order step: with e = 1 - x r0, |e| <= 2^-22,
+// r = r0 (1 + e + e^2) has relative error e^3 = 2^-66 (three dependent FMAs; two Newton steps need four).
 __device__ __forceinline__ double fast_rcp(double x)
 {
     const int hi = __double2hiint(x), lo = __double2loint(x);
@@ -540,18 +543,32 @@ __device__ __forceinline__ double fast_rcp(double x)
     const unsigned rb = __float_as_uint(rf);
     const int ex = (hi >> 20) & 0x7FF;
     const int rexp = (int)(rb >> 23) + (1023 - 127) - (ex - 1023);
-    double r = __hiloint2double((rexp << 20) | (int)((rb >> 3) & 0xFFFFF), (int)(rb << 29));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    return r;
+    const double r = __hiloint2double((rexp << 20) | (int)((rb >> 3) & 0xFFFFF), (int)(rb << 29));
+    const double e = fma(-x, r, 1.0);
+    return fma(r, fma(e, e, e), r);
+}
+// 2^-k for the biased exponent field of a positive normal w = m 2^k: an exact rescaling factor
+__device__ __forceinline__ double pow2_inv_of(double w)
+{
+    const int e = (__double2hiint(w) >> 20) & 0x7FF;
+    return __hiloint2double((2046 - e) << 20, 0);
 }
 
 
 // EXACT: nx is a multiple of M (every chunk is full: no per-row bounds checks).  The coefficients {a_i, c_i}
-// are staged in shared memory (one conflict-free LDS.128 per row, one pad slot per chunk).
-__host__ __device__ constexpr int k3_coef_slots(int nx, int M) { return nx + nx / M + 1; }
+// are staged in shared memory, chunk q at slots [q (M+1), q (M+1) + M]: one conflict-free LDS.128 per row.
+__host__ __device__ constexpr int k3_coef_slots(int nx, int M) { return (nx / M + 2) * (M + 1); }
+
+// Chunk boundaries.  With 64-byte tile rows (KW = 4) a quarter warp holds two chunks q, q+1 of the same four
+// systems; their rows i0 + r are M rows = a multiple of 128 bytes apart, i.e. on the same 16 banks (ncu: 4.2-way
+// conflicts on every tile access, 2000 of 5300 shared-memory wavefronts per tile).  SKEW = 1 starts the odd chunks
+// one row later (even chunks have M+1 rows, odd ones M-1), so that at every unrolled step the two chunks touch
+// rows of different parity = the two halves of the 32 banks.
+constexpr int K3_SKEW = 0;   // measured: 6 % slower with 1 (one more step on the dependent chain costs more than the conflicts)
+__host__ __device__ constexpr int k3_chunk_start(int q, int M, int skew, int nx, int pch)
+{
+    return q >= pch ? nx : ((q * M + skew * (q & 1) < nx - 1) ? q * M + skew * (q & 1) : nx - 1);
+}
 
 // rows per TMA box of the K3 tile gather (box = 8 ky x 1 kz x k3_box_rows(nx) planes), and the rows the
 // boxes cover together (>= nx; the excess is out of bounds in i and arrives as zeros)
@@ -577,6 +594,9 @@ __global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_consta
     const int kz = blockIdx.x / ntile, ky0 = (blockIdx.x % ntile) * KW;   // first ky of this CTA
     const int s = threadIdx.x % KW, q = threadIdx.x / KW;
     const int slot = q * KW + s, NS = PCH * KW;
+    constexpr int SK = (KW == 4) ? K3_SKEW : 0;    // skewed chunk starts (k3_chunk_start)
+    constexpr bool FULL = EXACT && SK == 0;        // every chunk has exactly M rows
+    constexpr int NI = M - 1 + SK;                 // most interior rows of a chunk
 
     // gather the 8 columns C[kz][0..nx)[8 kyt .. 8 kyt + 8): TMA boxes of 128-byte rows, one mbarrier
     if (threadIdx.x == 0) {
@@ -587,17 +607,25 @@ __global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_consta
     if (threadIdx.x == 0) {
         const int nb = k3_num_boxes(nx), br = k3_box_rows(nx);
         const unsigned long long pol = l2_policy((P.hints & 1) ? 1 : 0);
-        mbar_expect_tx(&bar, (uint32_t)(nb * br * KW * sizeof(cplx)));
+        // the coefficient table (already in the shared-memory layout) rides on the same mbarrier as the tile
+        const uint32_t coef_bytes = (uint32_t)(k3_coef_slots(nx, M) * sizeof(double2));
+        mbar_expect_tx(&bar, (uint32_t)(nb * br * KW * sizeof(cplx)) + coef_bytes);
         for (int b = 0; b < nb; ++b) tma_load_3d_hint(tile + (size_t)b * br * KW, &mapC, ky0 * 2, b * br, kz, &bar, pol);
+        bulk_load(coef, P.acp, coef_bytes, &bar);
+        // the tile of the CTA that will take this one's place on the SM: HBM -> L2 now, so that its gather is an L2 hit
+        const unsigned nxt = blockIdx.x + (unsigned)P.k3_prefetch;
+        if (P.k3_prefetch > 0 && nxt < gridDim.x) {
+            const int kz2 = nxt / ntile, ky2 = (nxt % ntile) * KW;
+            for (int b = 0; b < nb; ++b) tma_prefetch_3d(&mapC, ky2 * 2, b * br, kz2);
+        }
     }
-    for (int i = threadIdx.x; i < nx; i += blockDim.x) coef[i + i / M] = make_double2(__ldg(&P.ca[i]), __ldg(&P.cc[i]));
-    __syncthreads();
-    mbar_wait(&bar, 0);
-    auto ld_ac = [&](int i) -> double2 { return coef[i + i / M]; };   // {a_i, c_i}: one conflict-free LDS.128
     const double lam = __ldg(&P.lamy[ky0 + s]) + __ldg(&P.lamz[kz]);
+    mbar_wait(&bar, 0);
     const bool cta_singular = (blockIdx.x == 0) && P.has_mean;
-    const int i0 = q * M;
-    const int i1 = min(i0 + M, nx) - 1; // interface row of this chunk
+    const int i0 = k3_chunk_start(q, M, SK, nx, PCH);
+    const int i1 = k3_chunk_start(q + 1, M, SK, nx, PCH) - 1; // interface row of this chunk
+    const double2* mycoef = coef + q * (M + 1);
+    auto ld_ac = [&](int i) -> double2 { return mycoef[i - i0]; };   // {a_i, c_i}, i0 <= i <= i1: one conflict-free LDS.128
     double* bA = red;
     double* bC = red + NS;
     double* bL = red + 2 * NS;
@@ -609,7 +637,7 @@ __global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_consta
     double* nFr = nA + 3 * NS;
     double* nFi = nA + 4 * NS;
 
-    constexpr int MI = (M - 1 > 0) ? M - 1 : 1;
+    constexpr int MI = (NI > 0) ? NI : 1;
     double G[MI], H[MI];
     double rA, rC, rL, rFr, rFi;
     {   // ONE elimination sweep over the chunk interior, in place (tile <- y), one reciprocal per row:
@@ -618,23 +646,42 @@ __global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_consta
         // (Pg = g_0 ... g_{r-1}):   x_{i0} = Y + Gq E_q + Hq E_{q-1},
         //   Y = sum Pg y_r,  Hq = sum Pg h_r,  Gq = g_0 ... g_last,  Tq = 1 - Gq - Hq = sum Pg t_r  (no cancellation)
         // -- what the interface above needs for its reduced row, without a second (upward) elimination.
+        // The kernel is bound by the latency of this dependent chain (ncu: 16 warps per SM, short-scoreboard and
+        // fixed-latency stalls), so the pivots are carried UNNORMALISED: with W = the product of the pivots so far,
+        //   Hn = h W, Tn = t W, S = Hn + Tn, Yn = y W:
+        //   W <- (c + lam) W + a S,  S <- a S + lam W,  Hn <- a Hn,  Tn <- a Tn + lam W,  Yn <- a Yn + f W
+        // -- linear recurrences two operations deep, still sums of non-negatives (R9); the reciprocal of W and
+        // everything normalised by it (g = c W'/W, h, t, y) is off the chain.  W grows by at most the largest pivot
+        // per row; every 8 rows all carried quantities are rescaled by the exact power of two 2^-exponent(W).
+        double Hn = 1.0, Tn = 0.0, S = 1.0, W = 1.0, Ynr = 0.0, Yni = 0.0;
         double h = 1.0, t = 0.0, yr = 0.0, yi = 0.0;
         double Pg = 1.0, Yr = 0.0, Yi = 0.0, Hq = 0.0, Tq = 0.0;
 #pragma unroll
-        for (int r = 0; r < M - 1; ++r) {
+        for (int r = 0; r < NI; ++r) {
             const int i = i0 + r;
-            if (EXACT || i < i1) {
+            if (FULL || i < i1) {
+                if (r > 0 && r % 8 == 0) {
+                    const double sc = pow2_inv_of(W);
+                    W *= sc; S *= sc; Hn *= sc; Tn *= sc; Ynr *= sc; Yni *= sc;
+                }
                 const double2 ac = ld_ac(i);
                 const double a = ac.x, c = ac.y;
-                const double nh = a * h, nt = fma(a, t, lam);
-                const double rr = fast_rcp(c + (nh + nt));
                 const cplx f = tile[i * KW + s];
-                h = nh * rr;
-                t = nt * rr;
-                yr = fma(a, yr, f.x) * rr;
-                yi = fma(a, yi, f.y) * rr;
+                const double lw = lam * W;
+                const double Wn = fma(c + lam, W, a * S);
+                S = fma(a, S, lw);
+                Hn = a * Hn;
+                Tn = fma(a, Tn, lw);
+                Ynr = fma(a, Ynr, f.x * W);
+                Yni = fma(a, Yni, f.y * W);
+                const double rw = fast_rcp(Wn);
+                const double g = (c * W) * rw;
+                W = Wn;
+                h = Hn * rw;
+                t = Tn * rw;
+                yr = Ynr * rw;
+                yi = Yni * rw;
                 tile[i * KW + s] = mk(yr, yi);
-                const double g = c * rr;
                 G[r] = g;
                 H[r] = h;
                 Yr = fma(Pg, yr, Yr);
@@ -645,7 +692,7 @@ __global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_consta
             }
         }
         if (q > 0) { // contribution to the interface row above (reduced row q-1); staged in the "next" buffer
-            const double cb = coef[(i0 - 1) + (i0 - 1) / M].y;
+            const double cb = mycoef[-(M + 1) + (i0 - 1 - k3_chunk_start(q - 1, M, SK, nx, PCH))].y;   // c of the interface row above
             nC[slot - KW] = cb * Pg;
             nL[slot - KW] = cb * Tq;
             nFr[slot - KW] = cb * Yr;
@@ -670,28 +717,27 @@ __global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_consta
     if (cta_singular && s == 0 && q == PCH - 1) { // pin the last unknown of the mean mode
         rA = 0.0; rC = 0.0; rL = 1.0; rFr = 0.0; rFi = 0.0;
     }
-    // cancellation-free PCR over the PCH interface unknowns of each system
+    // cancellation-free PCR over the PCH interface unknowns of each system.  Every row publishes itself
+    // NORMALISED by its own diagonal (one reciprocal per row and level, before the exchange), so that the
+    // elimination factors al = A / D(q-d), ga = C / D(q+d) need no reciprocal after the loads.
     for (int d = 1; d < PCH; d <<= 1) {
-        bA[slot] = rA; bC[slot] = rC; bL[slot] = rL; bFr[slot] = rFr; bFi[slot] = rFi;
+        const double rD = fast_rcp(rA + rC + rL);
+        bA[slot] = rA * rD; bC[slot] = rC * rD; bL[slot] = rL * rD; bFr[slot] = rFr * rD; bFi[slot] = rFi * rD;
         __syncthreads();
         double A2 = 0.0, C2 = 0.0;
         if (q - d >= 0) {
             const int m = slot - KW * d;
-            const double Am = bA[m], Lm = bL[m];
-            const double al = rA * fast_rcp(Am + bC[m] + Lm);
-            A2 = al * Am;
-            rL = fma(al, Lm, rL);
-            rFr = fma(al, bFr[m], rFr);
-            rFi = fma(al, bFi[m], rFi);
+            A2 = rA * bA[m];
+            rL = fma(rA, bL[m], rL);
+            rFr = fma(rA, bFr[m], rFr);
+            rFi = fma(rA, bFi[m], rFi);
         }
         if (q + d < PCH) {
             const int m = slot + KW * d;
-            const double Cp = bC[m], Lp = bL[m];
-            const double ga = rC * fast_rcp(bA[m] + Cp + Lp);
-            C2 = ga * Cp;
-            rL = fma(ga, Lp, rL);
-            rFr = fma(ga, bFr[m], rFr);
-            rFi = fma(ga, bFi[m], rFi);
+            C2 = rC * bC[m];
+            rL = fma(rC, bL[m], rL);
+            rFr = fma(rC, bFr[m], rFr);
+            rFi = fma(rC, bFi[m], rFi);
         }
         rA = A2;
         rC = C2;
@@ -718,9 +764,9 @@ __global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_consta
         if (!cta_singular) {
             dst[i1 * 8 + s] = mk(xr, xi);
 #pragma unroll
-            for (int r = M - 2; r >= 0; --r) {
+            for (int r = NI - 1; r >= 0; --r) {
                 const int i = i0 + r;
-                if (EXACT || i < i1) {
+                if (FULL || i < i1) {
                     const cplx y = tile[i * KW + s];
                     xr = fma(G[r], xr, fma(H[r], elr, y.x));
                     xi = fma(G[r], xi, fma(H[r], eli, y.y));
@@ -731,9 +777,9 @@ __global__ void __launch_bounds__(TB) k_solve_x(DevParams P, const __grid_consta
         }
         tile[i1 * KW + s] = mk(xr, xi);
 #pragma unroll
-        for (int r = M - 2; r >= 0; --r) {
+        for (int r = NI - 1; r >= 0; --r) {
             const int i = i0 + r;
-            if (EXACT || i < i1) {
+            if (FULL || i < i1) {
                 const cplx y = tile[i * KW + s];
                 xr = fma(G[r], xr, fma(H[r], elr, y.x));
                 xi = fma(G[r], xi, fma(H[r], eli, y.y));

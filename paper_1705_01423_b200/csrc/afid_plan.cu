@@ -184,7 +184,7 @@ bool lookup_fft_z(int n, LaunchCfg* k1, LaunchCfg* k5)
 constexpr int MAX_NX = 2048;
 
 // K3 instantiation, block size and shared memory for nx rows
-LaunchCfg select_k3(int nx, int* kw_out)
+LaunchCfg select_k3(int nx, int* kw_out, int* m_out)
 {
     LaunchCfg c{};
     int M, kw = 8;
@@ -208,6 +208,7 @@ LaunchCfg select_k3(int nx, int* kw_out)
     c.ctas_per_sm = 4;
     c.nl = 0;
     *kw_out = kw;
+    *m_out = M;
     return c;
 }
 
@@ -376,7 +377,8 @@ static afid_plan* create_impl(int nx, int ny, int nz, const double* xc, double L
     pl->nx = nxl; pl->ny = ny; pl->nz = nz; pl->nzh = nh + 1;
 
     // ---- K3 configuration
-    pl->k3 = select_k3(nx, &pl->k3_kw);
+    int k3_m = 0;
+    pl->k3 = select_k3(nx, &pl->k3_kw, &k3_m);
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -428,6 +430,17 @@ static afid_plan* create_impl(int nx, int ny, int nz, const double* xc, double L
     fill_tw(twy, ny, ny);
     fill_tw(twzh, nh, nh);
     fill_tw(twz, nh + 1, nz);
+    // K3's coefficient table {a_i, c_i} in the kernel's shared-memory layout (one bulk copy per CTA)
+    std::vector<double> acp(2 * (size_t)k3_coef_slots(nx, k3_m), 0.0);
+    {
+        const int sk = (pl->k3_kw == 4) ? K3_SKEW : 0, pch = (nx + k3_m - 1) / k3_m;
+        for (int q = 0; q < pch; ++q)
+            for (int i = k3_chunk_start(q, k3_m, sk, nx, pch); i < k3_chunk_start(q + 1, k3_m, sk, nx, pch); ++i) {
+                const size_t slot = (size_t)q * (k3_m + 1) + (i - k3_chunk_start(q, k3_m, sk, nx, pch));
+                acp[2 * slot] = ca[i];
+                acp[2 * slot + 1] = cc[i];
+            }
+    }
 
     // ---- one device allocation for all tables (each sub-table 256-byte aligned)
     struct Item { const void* src; size_t bytes; size_t off; };
@@ -435,7 +448,7 @@ static afid_plan* create_impl(int nx, int ny, int nz, const double* xc, double L
         {rdx.data(), rdx.size() * 8, 0}, {rdc.data(), rdc.size() * 8, 0}, {dx.data(), dx.size() * 8, 0},
         {ca.data(), ca.size() * 8, 0},   {cc.data(), cc.size() * 8, 0},   {lamy.data(), lamy.size() * 8, 0},
         {lamz.data(), lamz.size() * 8, 0}, {twy.data(), twy.size() * 8, 0}, {twzh.data(), twzh.size() * 8, 0},
-        {twz.data(), twz.size() * 8, 0}};
+        {twz.data(), twz.size() * 8, 0}, {acp.data(), acp.size() * 8, 0}};
     size_t off = 0;
     for (auto& it : items) { it.off = off; off += (it.bytes + 255) / 256 * 256; }
     pl->tables_bytes = off;
@@ -479,9 +492,16 @@ static afid_plan* create_impl(int nx, int ny, int nz, const double* xc, double L
     d.tw_y = (const cplx*)(tb + items[7].off);
     d.tw_zh = (const cplx*)(tb + items[8].off);
     d.tw_z = (const cplx*)(tb + items[9].off);
+    d.acp = (const double2*)(tb + items[10].off);
     d.inv_vol = (double)(1.0L / vol);
     d.hints = 0;
     d.has_mean = (ks == 0) ? 1 : 0;
+    d.k3_prefetch = 0;
+    {   // K3 prefetch distance = the CTAs resident at once
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pl->k3.fn, pl->k3.threads, pl->k3.smem) == cudaSuccess && occ >= 1) d.k3_prefetch = occ * pl->n_sm;
+        else cudaGetLastError();
+    }
     pl->dps = d;                 // x-solve: all planes, this rank's kz
     pl->dps.nzh = nkz;
     pl->dps.lamz = d.lamz + ks;

@@ -66,6 +66,20 @@ __device__ __forceinline__ void tma_load_3d_hint(void* smem_dst, const CUtensorM
         : "memory");
 }
 
+// contiguous bulk load global -> shared (bytes: multiple of 16; both addresses 16-byte aligned), completion on an mbarrier
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)), "l"(gsrc),
+                 "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// prefetch of a 3-D tiled tensor box into L2 (no shared-memory destination, no completion)
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap* map, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
 // contiguous bulk store shared -> global (bytes: multiple of 16; both addresses 16-byte aligned)
 __device__ __forceinline__ void bulk_store(void* gdst, const void* smem_src, uint32_t bytes)
 {
