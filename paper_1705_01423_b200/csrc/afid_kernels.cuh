@@ -131,58 +131,45 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 256) ? 2 : 1) k_
     {
         typedef FftPass<PL, 0> P0;
         constexpr int R = P0::R, NB = P0::NB;
-        constexpr int NBATCH = (R % 4 == 0) ? 4 : (R % 3 == 0 ? 3 : (R % 2 == 0 ? 2 : 1));
+        // one batch = all five streams of NBATCH element pairs: 5 NBATCH 16-byte loads + NBATCH 8-byte loads in flight per
+        // thread, R / NBATCH round trips to memory per CTA (separate u, v, w batches of 8 loads needed 12 round trips for
+        // R = 16; ncu: the load phase is 46 % of the kernel, all of it long-scoreboard stalls at 12 warps per SM)
+        constexpr int NBATCH = (R % 2 == 0) ? 2 : 1;
         static_assert(P0::ROUNDS == 1, "K1 expects one first-pass butterfly per thread");
         typename P0::Regs rg;
         const bool act = P0::EXACT || tl < NB;
         if (act) {
 #pragma unroll
             for (int h = 0; h < R; h += NBATCH) {
-                double2 x1[NBATCH], x0[NBATCH];
-#pragma unroll
-                for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2h(u1 + 2 * (tl + NB * (h + r)), pol_u1); x0[r] = ldv2h(u0 + 2 * (tl + NB * (h + r)), pol_in); }
-                SCHED_FENCE();
-#pragma unroll
-                for (int r = 0; r < NBATCH; ++r) { pin(x1[r]); pin(x0[r]); }
-#pragma unroll
-                for (int r = 0; r < NBATCH; ++r) rg.v[0][h + r] = mk((x1[r].x - x0[r].x) * rdx, (x1[r].y - x0[r].y) * rdx);
-            }
-#pragma unroll
-            for (int h = 0; h < R; h += NBATCH) {
-                double2 x1[NBATCH], x0[NBATCH];
-#pragma unroll
-                for (int r = 0; r < NBATCH; ++r) { x1[r] = ldv2h(v1 + 2 * (tl + NB * (h + r)), pol_u1); x0[r] = ldv2h(v0 + 2 * (tl + NB * (h + r)), pol_in); }
-                SCHED_FENCE();
-#pragma unroll
-                for (int r = 0; r < NBATCH; ++r) { pin(x1[r]); pin(x0[r]); }
-#pragma unroll
-                for (int r = 0; r < NBATCH; ++r) {
-                    rg.v[0][h + r].x = fma(x1[r].x - x0[r].x, rdy, rg.v[0][h + r].x);
-                    rg.v[0][h + r].y = fma(x1[r].y - x0[r].y, rdy, rg.v[0][h + r].y);
-                }
-            }
-#pragma unroll
-            for (int h = 0; h < R; h += NBATCH) {
-                double2 x0[NBATCH];
+                double2 a1[NBATCH], a0[NBATCH], b1[NBATCH], b0[NBATCH], c0[NBATCH];
                 double cn[NBATCH];
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) {
                     const int e = tl + NB * (h + r);
-                    x0[r] = ldv2h(w0 + 2 * e, pol_in);
+                    a1[r] = ldv2h(u1 + 2 * e, pol_u1);
+                    a0[r] = ldv2h(u0 + 2 * e, pol_in);
+                    b1[r] = ldv2h(v1 + 2 * e, pol_u1);
+                    b0[r] = ldv2h(v0 + 2 * e, pol_in);
+                    c0[r] = ldv2h(w0 + 2 * e, pol_in);
                     cn[r] = ldv1h(w0 + ((e == Nh - 1) ? 0 : 2 * e + 2), pol_in);
                 }
                 SCHED_FENCE();
 #pragma unroll
-                for (int r = 0; r < NBATCH; ++r) { pin(x0[r]); pin1(cn[r]); }
+                for (int r = 0; r < NBATCH; ++r) { pin(a1[r]); pin(a0[r]); pin(b1[r]); pin(b0[r]); pin(c0[r]); pin1(cn[r]); }
 #pragma unroll
                 for (int r = 0; r < NBATCH; ++r) {
-                    rg.v[0][h + r].x = fma(x0[r].y - x0[r].x, rdz, rg.v[0][h + r].x);
-                    rg.v[0][h + r].y = fma(cn[r] - x0[r].y, rdz, rg.v[0][h + r].y);
+                    double dx_ = (a1[r].x - a0[r].x) * rdx, dy_ = (a1[r].y - a0[r].y) * rdx;
+                    dx_ = fma(b1[r].x - b0[r].x, rdy, dx_);
+                    dy_ = fma(b1[r].y - b0[r].y, rdy, dy_);
+                    dx_ = fma(c0[r].y - c0[r].x, rdz, dx_);
+                    dy_ = fma(cn[r] - c0[r].y, rdz, dy_);
+                    rg.v[0][h + r] = mk(dx_, dy_);
                 }
             }
             P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { line[PL::pad(e)] = val; });
         }
     }
+    constexpr int SPLIT_N = (Nh / 2 + 1) * NL;
     {   // barriers between the passes only over the warps of a line group (see K5); the split below needs all lines
         constexpr int GL = (TPL % 32 == 0) ? 1 : ((2 * TPL) % 32 == 0 ? 2 : 4);
         if constexpr (GL < NL && (GL * TPL) % 32 == 0) {
@@ -199,14 +186,18 @@ __global__ void __launch_bounds__(NL* PL::TPL, (NL * PL::TPL <= 256) ? 2 : 1) k_
     // B may be a rotating buffer of bmod planes (plane-batched launches keep it L2-resident)
     cplx* out = B + ((size_t)(i % bmod) * (P.ny / 8) + (size_t)(jg * NL / 8)) * (size_t)P.nzh * 8;
     const double hs = 0.5 * P.spec_scale;
-    for (int idx = threadIdx.x; idx < (Nh / 2 + 1) * NL; idx += NL * TPL) {
+    // the twiddle of the NEXT iteration is always in flight (ncu: the load -> use latency inside this loop was 7 % of
+    // the kernel's stall samples)
+    cplx wk_next = __ldg(&P.tw_z[min((int)threadIdx.x, SPLIT_N - 1) / NL]);
+    for (int idx = threadIdx.x; idx < SPLIT_N; idx += NL * TPL) {
         const int k = idx / NL, l = idx % NL;
         const cplx* zl = sm + l * LS;
         const cplx zk = zl[PL::pad(k)];
         const cplx zm = zl[PL::pad(k == 0 ? 0 : Nh - k)];
         // E = Z(k) + conj Z(Nh-k);  O = Z(k) - conj Z(Nh-k)
         const cplx E = mk(zk.x + zm.x, zk.y - zm.y), O = mk(zk.x - zm.x, zk.y + zm.y);
-        const cplx wk = __ldg(&P.tw_z[k]); // exp(-2 pi i k / nz)
+        const cplx wk = wk_next; // exp(-2 pi i k / nz)
+        if (idx + NL * TPL < SPLIT_N) wk_next = __ldg(&P.tw_z[(idx + NL * TPL) / NL]);
         // -i w O
         const cplx wo = cmul(wk, O);
         const cplx t = mk(wo.y, -wo.x);
@@ -337,24 +328,30 @@ template <class PL> constexpr int k5_smem_rows()
 // step is gathered by TMA into the other buffer while this one is transformed, so HBM always has a request of
 // this SM in flight (the non-persistent version waited for its whole tile before doing anything: 17 % of its
 // stall samples).  A buffer is handed back to the async proxy (TMA writes) after a proxy fence and a CTA barrier.
-template <class PL, int LPR, int NBUF>
+// STW: the pre-processing twiddles exp(-2 pi i k / nz) are staged in shared memory (wherever they fit beside the tiles)
+template <class PL, int LPR, int NBUF, bool STW>
 __global__ void __launch_bounds__(LPR* PL::TPL, 1) k_c2r_z(DevParams P, const __grid_constant__ CUtensorMap mapD, double* __restrict__ p, int i_base, int np,
                                                            int dmod)
 {
-    constexpr int Nh = PL::N, TPL = PL::TPL, NL = 8;
+    constexpr int Nh = PL::N, TPL = PL::TPL, NL = 8, NT = LPR * TPL;
     constexpr int TILE = k5_smem_rows<PL>() * 8;     // complex slots per buffer
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t bar[NBUF];
+    __shared__ __align__(8) uint64_t bar[NBUF];      // "full": the TMA gather of a buffer has landed
+    __shared__ __align__(8) uint64_t empty[NBUF];    // "empty": every thread is done with the buffer's shared memory
     // 1024-byte aligned tiles [row][8 chunks of 16 bytes]; line l, row r lives in chunk l ^ (r & 7)
     // (the 128-byte TMA swizzle, kept for the in-place FFT passes: conflict-free for unit-stride rows)
     cplx* sm0 = reinterpret_cast<cplx*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u)); // (offset form keeps the shared state space)
+    cplx* stw = sm0 + (size_t)NBUF * TILE;           // exp(-2 pi i k / nz), k = 0..Nh: the pre-processing twiddles (ncu: their global loads
+                                                     // were 6 % of the stall samples; the persistent CTA stages them once)
     const int njt = P.ny / 8;
     const int ntile = np * njt;
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int b = 0; b < NBUF; ++b) mbar_init(&bar[b], 1);
+        for (int b = 0; b < NBUF; ++b) { mbar_init(&bar[b], 1); mbar_init(&empty[b], NT); }
         fence_mbar_init();
     }
+    if constexpr (STW)
+        for (int k = threadIdx.x; k <= Nh; k += NT) stw[k] = __ldg(&P.tw_z[k]);
     __syncthreads();
     const unsigned long long pol = l2_policy((P.hints & 4) ? 1 : ((P.hints & 2) ? 2 : 0));
     auto issue = [&](int t, int buf) {   // one thread: gather tile t into buffer buf
@@ -378,7 +375,11 @@ __global__ void __launch_bounds__(LPR* PL::TPL, 1) k_c2r_z(DevParams P, const __
 #pragma unroll 1
     for (int t = blockIdx.x; t < ntile; t += gridDim.x, ++n) {
         const int buf = (NBUF == 2) ? (n & 1) : 0;
-        if (NBUF == 2 && threadIdx.x == 0 && t + (int)gridDim.x < ntile) issue(t + gridDim.x, buf ^ 1);
+        if (NBUF == 2 && threadIdx.x == 0 && t + (int)gridDim.x < ntile) {
+            // the other buffer held the tile of step n-1: wait until all threads have handed it back (its use number (n-1)/2)
+            if (n >= 1) mbar_wait(&empty[buf ^ 1], (uint32_t)(((n - 1) >> 1) & 1));
+            issue(t + gridDim.x, buf ^ 1);
+        }
         cplx* sm = sm0 + (size_t)buf * TILE;
         const int i = i_base + t / njt, jt = t % njt;
         auto at = [sm](int l, int r) -> cplx& { return sm[(r << 3) + (l ^ (r & 7))]; };
@@ -390,7 +391,7 @@ __global__ void __launch_bounds__(LPR* PL::TPL, 1) k_c2r_z(DevParams P, const __
             const int k = min(e, Nh - e), km = Nh - k;
             const cplx xk = at(l, k);
             const cplx xm = at(l, km);
-            const cplx wk = __ldg(&P.tw_z[k]);
+            const cplx wk = STW ? stw[k] : __ldg(&P.tw_z[k]);
             const cplx E = mk(xk.x + xm.x, xk.y - xm.y), O = mk(xk.x - xm.x, xk.y + xm.y);
             const cplx wo = mk(fma(wk.y, O.y, wk.x * O.x), fma(-wk.y, O.x, wk.x * O.y)); // conj(w) * O
             const cplx tt = mk(-wo.y, wo.x);                                             // i conj(w) O
@@ -399,26 +400,38 @@ __global__ void __launch_bounds__(LPR* PL::TPL, 1) k_c2r_z(DevParams P, const __
 #pragma unroll 1
         for (int rnd = 0; rnd < NL / LPR; ++rnd) {
             const int ln = rnd * LPR + lr;
+            const bool last_round = (rnd == NL / LPR - 1);
             double* dst = p + ((size_t)i * P.ny + (size_t)jt * 8 + ln) * (size_t)P.nz;
             auto st_p = [&](int e, cplx val) { reinterpret_cast<double2*>(dst)[e] = cswap(val); };
             auto acc = [sm, ln](int pe) -> cplx& { return sm[(pe << 3) + (ln ^ (pe & 7))]; };
+            // after the last shared-memory read of the tile (before the global stores of p): hand the buffer back to the
+            // TMA (async proxy).  Only the issuing thread ever waits for it (at the top of the next step), so nobody
+            // stalls on the stores (ncu: the fence + CTA barrier after the stores were 11 % of the stall samples).
+            auto release = [&]() {
+                if (NBUF == 2 && last_round) {
+                    fence_proxy_async();
+                    mbar_arrive(&empty[buf]);
+                }
+            };
             typedef FftPass<PL, 0> P0;
             {
                 typename P0::Regs rg;
                 P0::load(rg, tl, [&](int e) { return zprime(ln, e); });   // unpadded rows, as TMA delivered them
                 if constexpr (PL::NPASS == 1) {
+                    release();
                     P0::compute_store(rg, tl, P.tw_zh, st_p);
                 } else {
                     sync();
                     P0::compute_store(rg, tl, P.tw_zh, [&](int e, cplx val) { acc(PL::pad(e)) = val; });
                 }
             }
-            if constexpr (PL::NPASS > 1) fft_tail_passes_acc<PL, 1, false>(acc, tl, true, P.tw_zh, st_p, sync);
+            if constexpr (PL::NPASS > 1) fft_tail_passes_acc<PL, 1, false>(acc, tl, true, P.tw_zh, st_p, sync, release);
         }
-        // this buffer goes back to the TMA (async proxy) at the next step (NBUF = 1) or the one after (NBUF = 2)
-        fence_proxy_async();
-        __syncthreads();
-        if (NBUF == 1 && threadIdx.x == 0 && t + (int)gridDim.x < ntile) issue(t + gridDim.x, 0);
+        if (NBUF == 1) {   // one buffer: it goes back to the TMA once every thread has passed this point
+            fence_proxy_async();
+            __syncthreads();
+            if (threadIdx.x == 0 && t + (int)gridDim.x < ntile) issue(t + gridDim.x, 0);
+        }
     }
 }
 

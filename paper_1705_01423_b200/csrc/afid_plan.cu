@@ -140,12 +140,16 @@ template <class PL> LaunchCfg cfg_k4()
 // K5: all 8 lines of a tile in one round where that leaves >= 128 registers per thread, else two rounds of 4;
 // two tile buffers (TMA prefetch of the next tile) where they fit the 227 KB of an SM
 template <class PL> constexpr int k5_lpr() { return (8 * PL::TPL <= 512) ? 8 : 4; }
-template <class PL> constexpr int k5_nbuf() { return (2 * (size_t)k5_smem_rows<PL>() * 8 * sizeof(cplx) + 2048 <= 227 * 1024) ? 2 : 1; }
+// bytes of K5's staged twiddle table (nz/2 + 1 complex, rounded up to 128 bytes)
+template <class PL> constexpr size_t k5_tw_bytes() { return ((size_t)(PL::N + 1) * sizeof(cplx) + 127) / 128 * 128; }
+template <class PL> constexpr size_t k5_tile_bytes() { return (size_t)k5_smem_rows<PL>() * 8 * sizeof(cplx); }
+template <class PL> constexpr int k5_nbuf() { return (2 * k5_tile_bytes<PL>() + 2048 <= 227 * 1024) ? 2 : 1; }
+template <class PL> constexpr bool k5_stw() { return k5_nbuf<PL>() * k5_tile_bytes<PL>() + k5_tw_bytes<PL>() + 2048 <= 227 * 1024; }
 template <class PL> LaunchCfg cfg_k5()
 {
     // .nl = CTAs per SM the launch is sized for
-    return {(const void*)k_c2r_z<PL, k5_lpr<PL>(), k5_nbuf<PL>()>, k5_lpr<PL>() * PL::TPL,
-            (size_t)k5_nbuf<PL>() * k5_smem_rows<PL>() * 8 * sizeof(cplx) + 1024, 1, 1};
+    return {(const void*)k_c2r_z<PL, k5_lpr<PL>(), k5_nbuf<PL>(), k5_stw<PL>()>, k5_lpr<PL>() * PL::TPL,
+            k5_nbuf<PL>() * k5_tile_bytes<PL>() + (k5_stw<PL>() ? k5_tw_bytes<PL>() : 0) + 1024, 1, 1};
 }
 
 bool lookup_fft_y(int n, LaunchCfg* k2, LaunchCfg* k4)

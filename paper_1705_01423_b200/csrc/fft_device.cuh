@@ -257,8 +257,14 @@ struct GroupSync {
     __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 };
 
-template <class PL, int P, bool LAST_TO_SMEM, class Acc, class StoreLast, class Sync = CtaSync>
-__device__ __forceinline__ void fft_tail_passes_acc(Acc acc, int tl, bool active, const cplx* __restrict__ tw, StoreLast st_last, Sync sync = Sync())
+struct NoHook {
+    __device__ __forceinline__ void operator()() const {}
+};
+// `loaded()` is called once, right after the loads of the LAST pass (the line's shared-memory slots are dead from
+// then on: a kernel that recycles the buffer can hand it back before the global stores).
+template <class PL, int P, bool LAST_TO_SMEM, class Acc, class StoreLast, class Sync = CtaSync, class Hook = NoHook>
+__device__ __forceinline__ void fft_tail_passes_acc(Acc acc, int tl, bool active, const cplx* __restrict__ tw, StoreLast st_last, Sync sync = Sync(),
+                                                    Hook loaded = Hook())
 {
     if constexpr (P < PL::NPASS) {
         typedef FftPass<PL, P> PS;
@@ -266,12 +272,13 @@ __device__ __forceinline__ void fft_tail_passes_acc(Acc acc, int tl, bool active
         sync(); // previous pass's writes visible
         if (active) PS::load(rg, tl, [&](int e) { return acc(PL::pad(e)); });
         if constexpr (P == PL::NPASS - 1 && !LAST_TO_SMEM) {
+            loaded();
             if (active) PS::compute_store(rg, tl, tw, st_last);
         } else {
             sync(); // all reads done before the in-place writes
             if (active) PS::compute_store(rg, tl, tw, [&](int e, cplx v) { acc(PL::pad(e)) = v; });
         }
-        fft_tail_passes_acc<PL, P + 1, LAST_TO_SMEM>(acc, tl, active, tw, st_last, sync);
+        fft_tail_passes_acc<PL, P + 1, LAST_TO_SMEM>(acc, tl, active, tw, st_last, sync, loaded);
     } else {
         if constexpr (LAST_TO_SMEM) sync();
     }

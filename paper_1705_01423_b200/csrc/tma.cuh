@@ -26,6 +26,11 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+// plain arrival (release): a consumer hands a buffer back
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 // wait for the phase with the given parity; traps instead of spinning forever if the copy never
 // completes (a wrong byte count or a bad tensor map must not hang the device)
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
