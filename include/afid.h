@@ -95,6 +95,17 @@ int afid_project(afid_plan* plan, double* u, double* v, double* w, double* p, vo
 int afid_max_cfl(afid_plan* plan, const double* u, const double* v, const double* w, double* cfl, void* stream);
 
 /*
+ * afid_project_cfl -- SURVEY.md 8(f3), fused form: afid_project, and the maximum CFL number (afid_max_cfl's
+ * definition, Listing 1) of the CORRECTED field into *cfl, taken inside the correction launch:
+ * the corrected u, v, w are reduced while they are still in L2 instead of being read back from HBM by a
+ * second pass (24 B per point).  Same arguments as afid_project plus cfl (DEVICE pointer to one double,
+ * 8-byte aligned, overwritten).  u, v, w, p come out bit-identical to afid_project's, and *cfl bit-identical
+ * to afid_max_cfl on them.  Enqueue only (one memset, five kernels + two small ones); capturable in a CUDA
+ * graph.  Unsharded plans only; not available with afid_plan_set_pipeline.
+ */
+int afid_project_cfl(afid_plan* plan, double* u, double* v, double* w, double* p, double* cfl, void* stream);
+
+/*
  * afid_plan_set_accumulate -- SURVEY.md 8(f3): choose what afid_project does with p.
  *   on = 0 (default)  p  = phi   (p is output only; its dx-weighted mean is zero; R6)
  *   on = 1            p += phi   (the "delta form" pressure update of the fractional step, P:L91, P:L116;

@@ -23,7 +23,7 @@ SYMBOLS = ["afid_plan_create", "afid_project", "afid_plan_destroy", "afid_plan_w
            "afid_plan_num_launches", "afid_stage_forward", "afid_stage_solve", "afid_fft_length_supported",
            "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version",
            "afid_plan_enable_timing", "afid_plan_kernel_times", "afid_plan_kernel_name",
-           "afid_fft_half_length_supported", "afid_max_cfl", "afid_plan_set_accumulate", "afid_xsolve_create", "afid_xsolve_apply",
+           "afid_fft_half_length_supported", "afid_max_cfl", "afid_project_cfl", "afid_plan_set_accumulate", "afid_xsolve_create", "afid_xsolve_apply",
            "afid_xsolve_destroy", "afid_plan_set_pipeline", "afid_plan_set_l2_hints", "afid_plan_num_timed",
            "afid_shard_plan_create", "afid_shard_bounds", "afid_shard_layout", "afid_shard_buffers", "afid_shard_info",
            "afid_shard_forward", "afid_shard_solve", "afid_shard_inverse", "afid_shard_correct"]
@@ -68,6 +68,8 @@ def lib():
         L.afid_xsolve_destroy.argtypes = [vp]
         L.afid_plan_set_accumulate.restype = i
         L.afid_plan_set_accumulate.argtypes = [vp, i]
+        L.afid_project_cfl.restype = i
+        L.afid_project_cfl.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.afid_max_cfl.restype = i
         L.afid_max_cfl.argtypes = [vp, vp, vp, vp, vp, vp]
         L.afid_fft_length_supported.restype = i
@@ -182,6 +184,17 @@ class Plan:
         n = self.nx * self.ny * self.nz
         _check(lib().afid_project(self._h, _dev_ptr(u, n + self.ny * self.nz, "u"), _dev_ptr(v, n, "v"),
                                   _dev_ptr(w, n, "w"), _dev_ptr(p, n, "p"), self._stream(stream)))
+
+    def project_cfl(self, u, v, w, p, out=None, stream=None):
+        """afid_project_cfl: afid_project plus the maximum CFL number of the corrected field, reduced inside the
+        correction launch, into a 1-element fp64 CUDA tensor (enqueued, no sync)."""
+        import torch
+        n = self.nx * self.ny * self.nz
+        if out is None:
+            out = torch.empty(1, dtype=torch.float64, device=u.device)
+        _check(lib().afid_project_cfl(self._h, _dev_ptr(u, n + self.ny * self.nz, "u"), _dev_ptr(v, n, "v"),
+                                      _dev_ptr(w, n, "w"), _dev_ptr(p, n, "p"), _dev_ptr(out, 1, "cfl"), self._stream(stream)))
+        return out
 
     def stage_forward(self, u, v, w, spec, stream=None):
         """afid_stage_forward: spec (fp64 tensor of 2*nx*nzh*ny, complex [i][kz][ky]) <- -(D u)^/(ny nz)."""

@@ -442,26 +442,12 @@ __global__ void __launch_bounds__(LPR* PL::TPL, 1) k_c2r_z(DevParams P, const __
 // ------------------------------------------------------------------------------------------
 constexpr int K6_JL = 4, K6_TX = 64, K6_U = 4;
 
-__global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const double* __restrict__ p, double* __restrict__ u,
-                                                          double* __restrict__ v, double* __restrict__ w, int i_base, int np, double* __restrict__ pacc,
-                                                          const double* __restrict__ p_halo)
+// the correction of the lines (i, JL jg .. JL jg + JL - 1); called by all K6_JL x K6_TX threads of a CTA
+__device__ __forceinline__ void k6_correct_item(const DevParams& P, const double* __restrict__ p, double* __restrict__ u, double* __restrict__ v,
+                                                double* __restrict__ w, int i, int jg, double* __restrict__ pacc, const double* __restrict__ p_halo,
+                                                unsigned long long pol_in, unsigned long long pol_out)
 {
-    // `p` holds phi; if pacc != nullptr the pressure is accumulated as well: pacc += phi (P:L91, P:L116 delta form).
-    // p_halo (sharded plans, SURVEY.md 8(f2)): the plane of phi below this slab's first plane (nullptr: plane 0 is the wall)
     constexpr int JL = K6_JL, TX = K6_TX, U = K6_U;
-    // this launch covers planes i_base .. i_base+np-1.
-    // CTA order: j-chunks of 32 lines outermost, then i, then the group inside the chunk, so that
-    // plane i-1 of p (read again for the x-gradient) is still in L2 when plane i is processed
-    const int ngrp = P.ny / JL;
-    constexpr int JC = 32 / JL;
-    const int per_chunk = np * JC;
-    int i, jg;
-    {
-        const int chunk = blockIdx.x / per_chunk, rem = blockIdx.x % per_chunk;
-        const int jc_here = min(JC, ngrp - chunk * JC);
-        i = i_base + rem / jc_here;
-        jg = chunk * JC + rem % jc_here;
-    }
     const int j = jg * JL + threadIdx.y;
     const int jm = (j == 0) ? P.ny - 1 : j - 1;
     const size_t plane = (size_t)P.ny * P.nz;
@@ -473,7 +459,6 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const dou
     const int nzh2 = P.nz / 2;
     const bool has_u = (i >= 1) || (p_halo != nullptr);
     const double rdc = has_u ? __ldg(&P.rdc[i]) : 0.0, rdy = P.rdy, rdz = P.rdz;
-    const unsigned long long pol_in = l2_policy((P.hints & 1) ? 1 : 0), pol_out = l2_policy((P.hints & 8) ? 1 : 0);
     for (int k0 = threadIdx.x; k0 < nzh2; k0 += TX * U) {
         double2 ph[U], pj[U], pi[U], uu[U], vv[U], ww[U];
         double pk[U];
@@ -517,6 +502,36 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const dou
             }
         }
     }
+}
+
+// item s of the CTA order of K6 -> (plane i, line group jg): j-chunks of JC groups outermost, then i, then the group inside
+// the chunk, so that plane i-1 of p (read again for the x-gradient) is still in L2 when plane i is processed
+constexpr int K6_JC = 32 / K6_JL;
+__device__ __forceinline__ void k6_item_to_ij(int s, int np, int ngrp, int& i, int& jg)
+{
+    const int per_chunk = np * K6_JC;
+    const int chunk = s / per_chunk, rem = s % per_chunk;
+    const int jc_here = min(K6_JC, ngrp - chunk * K6_JC);
+    i = rem / jc_here;
+    jg = chunk * K6_JC + rem % jc_here;
+}
+__device__ __forceinline__ int k6_ij_to_item(int i, int jg, int np, int ngrp)
+{
+    const int chunk = jg / K6_JC;
+    const int jc_here = min(K6_JC, ngrp - chunk * K6_JC);
+    return chunk * np * K6_JC + i * jc_here + (jg - chunk * K6_JC);
+}
+
+__global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const double* __restrict__ p, double* __restrict__ u,
+                                                          double* __restrict__ v, double* __restrict__ w, int i_base, int np, double* __restrict__ pacc,
+                                                          const double* __restrict__ p_halo)
+{
+    // `p` holds phi; if pacc != nullptr the pressure is accumulated as well: pacc += phi (P:L91, P:L116 delta form).
+    // p_halo (sharded plans, SURVEY.md 8(f2)): the plane of phi below this slab's first plane (nullptr: plane 0 is the wall)
+    // this launch covers planes i_base .. i_base+np-1.
+    int i, jg;
+    k6_item_to_ij((int)blockIdx.x, np, P.ny / K6_JL, i, jg);
+    k6_correct_item(P, p, u, v, w, i_base + i, jg, pacc, p_halo, l2_policy((P.hints & 1) ? 1 : 0), l2_policy((P.hints & 8) ? 1 : 0));
 }
 
 // ------------------------------------------------------------------------------------------
@@ -973,22 +988,27 @@ __device__ __forceinline__ unsigned long long cfl_bits(double q)   // q >= 0 or 
 __device__ __forceinline__ unsigned long long umax64(unsigned long long a, unsigned long long b) { return a > b ? a : b; }
 __global__ void k_cfl_init(double* __restrict__ cfl) { *cfl = 0.00000001; }
 
-__global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const double* __restrict__ u, const double* __restrict__ v,
-                                                          const double* __restrict__ w, double* __restrict__ cfl)
+__device__ __forceinline__ double2 ldcg2(const double* p)   // L2 only: data another SM wrote during this launch
 {
-    constexpr int JL = K6_JL, TX = K6_TX, U = K6_U;
-    __shared__ unsigned long long s_max[JL * TX / 32];
-    const int ngrp = P.ny / JL;
-    constexpr int JC = 32 / JL;
-    const int per_chunk = P.nx * JC;
-    int i, jg;
-    {
-        const int chunk = blockIdx.x / per_chunk, rem = blockIdx.x % per_chunk;
-        const int jc_here = min(JC, ngrp - chunk * JC);
-        i = rem / jc_here;
-        jg = chunk * JC + rem % jc_here;
-    }
-    const int j = jg * JL + threadIdx.y;
+    double2 r;
+    asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ double ldcg1(const double* p)
+{
+    double r;
+    asm volatile("ld.global.cg.f64 %0, [%1];" : "=d"(r) : "l"(p));
+    return r;
+}
+
+// Listing 1 over the cells of ONE line (i, j, all k) per thread row: thread x takes the cell pairs kp = x, x + TX, ...
+// in batches of U.  Returns the bit pattern of the thread's maximum.  CG: the loads bypass L1 (the fused kernel reads
+// what other SMs wrote a moment ago; L1 may still hold the uncorrected lines).
+template <bool CG>
+__device__ __forceinline__ unsigned long long cfl_line(const DevParams& P, const double* __restrict__ u, const double* __restrict__ v,
+                                                       const double* __restrict__ w, int i, int j)
+{
+    constexpr int TX = K6_TX, U = K6_U;
     const int jp = (j + 1 == P.ny) ? 0 : j + 1;
     const size_t plane = (size_t)P.ny * P.nz;
     const size_t ol = ((size_t)i * P.ny + j) * P.nz;
@@ -996,6 +1016,8 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const dou
     const double* vp = v + ((size_t)i * P.ny + jp) * P.nz;
     const int nzh2 = P.nz / 2;
     const double rdx = __ldg(&P.rdx[i]), rdy = P.rdy, rdz = P.rdz;
+    auto ld2 = [](const double* q) -> double2 { return CG ? ldcg2(q) : ldg2(q); };
+    auto ld1 = [](const double* q) -> double { return CG ? ldcg1(q) : __ldg(q); };
     unsigned long long best = 0ull;
     for (int k0 = threadIdx.x; k0 < nzh2; k0 += TX * U) {
         double2 u0[U], u1[U], v0[U], v1[U], w0[U];
@@ -1004,12 +1026,12 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const dou
         for (int r = 0; r < U; ++r) {
             const int kp = k0 + r * TX;
             if (kp < nzh2) {
-                u0[r] = ldg2(ul + 2 * kp);
-                u1[r] = ldg2(ul + plane + 2 * kp);
-                v0[r] = ldg2(vl + 2 * kp);
-                v1[r] = ldg2(vp + 2 * kp);
-                w0[r] = ldg2(wl + 2 * kp);
-                wn[r] = __ldg(wl + (kp == nzh2 - 1 ? 0 : 2 * kp + 2));
+                u0[r] = ld2(ul + 2 * kp);
+                u1[r] = ld2(ul + plane + 2 * kp);
+                v0[r] = ld2(vl + 2 * kp);
+                v1[r] = ld2(vp + 2 * kp);
+                w0[r] = ld2(wl + 2 * kp);
+                wn[r] = ld1(wl + (kp == nzh2 - 1 ? 0 : 2 * kp + 2));
             }
         }
 #pragma unroll
@@ -1022,14 +1044,108 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const dou
             }
         }
     }
+    return best;
+}
+// maximum over the CTA, one atomicMax on the bit pattern (s_max: one slot per warp; the caller synchronises before reuse)
+__device__ __forceinline__ void cfl_block_max(unsigned long long best, unsigned long long* s_max, double* __restrict__ cfl)
+{
 #pragma unroll
     for (int d = 16; d >= 1; d >>= 1) best = umax64(best, __shfl_xor_sync(0xffffffffu, best, d));
-    const int tid = threadIdx.y * TX + threadIdx.x;
+    const int tid = threadIdx.y * K6_TX + threadIdx.x;
     if ((tid & 31) == 0) s_max[tid >> 5] = best;
     __syncthreads();
     if (tid == 0) {
-        for (int k = 1; k < JL * TX / 32; ++k) best = umax64(best, s_max[k]);
+        for (int k = 1; k < K6_JL * K6_TX / 32; ++k) best = umax64(best, s_max[k]);
         atomicMax(reinterpret_cast<unsigned long long*>(cfl), best);
+    }
+}
+
+__global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const double* __restrict__ u, const double* __restrict__ v,
+                                                          const double* __restrict__ w, double* __restrict__ cfl)
+{
+    __shared__ unsigned long long s_max[K6_JL * K6_TX / 32];
+    int i, jg;
+    k6_item_to_ij((int)blockIdx.x, P.nx, P.ny / K6_JL, i, jg);
+    cfl_block_max(cfl_line<false>(P, u, v, w, i, jg * K6_JL + threadIdx.y), s_max, cfl);
+}
+
+// ------------------------------------------------------------------------------------------
+// SURVEY.md 8(f3), fused form: the correction (K6) with Listing 1's maximum taken over the CORRECTED field in
+// the same launch -- no second pass over u, v, w through HBM.  A cell's value needs the corrected u(i+1), v(j+1),
+// w(k+1), which belong to other CTAs' lines and are overwritten in place, so the reduction cannot ride in the
+// correcting CTA's registers.  Instead one persistent launch hands out tickets: ticket t corrects item t (the
+// CTA order of k_correct) and then reduces the cells of item t - lag, whose lines were corrected `lag` tickets
+// ago and are still in L2 (lag = resident CTAs + 16 items: < 50 MB of u, v, w at C4).  The reduce step owns the
+// lines JL jg - 1 .. JL jg + JL - 2 (one line down, so that v(j+1) stays inside the chunk that was just
+// corrected; the last group also takes line ny - 1, whose neighbour is line 0) and waits for the "done" flags
+// of the (at most five) items that wrote what it reads.  Every wait is for an EARLIER ticket, whose correction
+// part never waits: no deadlock whatever order the CTAs are scheduled in.  sync[0] = ticket counter,
+// sync[1 + s] = item s corrected (both zeroed by the host before the launch).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int ld_acquire_i32(const int* p)
+{
+    int r;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(r) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st_release_i32(int* p, int v) { asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory"); }
+
+__global__ void __launch_bounds__(K6_JL* K6_TX) k_correct_cfl(DevParams P, const double* __restrict__ p, double* __restrict__ u, double* __restrict__ v,
+                                                              double* __restrict__ w, double* __restrict__ pacc, double* __restrict__ cfl, int* __restrict__ sync,
+                                                              int lag)
+{
+    constexpr int JL = K6_JL, TX = K6_TX;
+    __shared__ unsigned long long s_max[JL * TX / 32];
+    __shared__ int s_tk;
+    const int tid = threadIdx.y * TX + threadIdx.x;
+    const int ngrp = P.ny / JL, nitems = P.nx * ngrp;
+    int* done = sync + 1;
+    const unsigned long long pol_in = l2_policy((P.hints & 4) ? 0 : 1), pol_out = l2_policy((P.hints & 2) ? 2 : 0);   // the uncorrected u, v, w are read once: evict first
+    int nxt = 0;
+    if (tid == 0) nxt = atomicAdd(&sync[0], 1);
+#pragma unroll 1
+    for (;;) {
+        if (tid == 0) {
+            s_tk = nxt;
+            nxt = atomicAdd(&sync[0], 1);   // the next ticket is fetched one item ahead: its latency hides behind this item
+        }
+        __syncthreads();
+        const int tk = s_tk;
+        if (tk >= nitems + lag) break;
+        if (tk < nitems) {
+            int i, jg;
+            k6_item_to_ij(tk, P.nx, ngrp, i, jg);
+            k6_correct_item(P, p, u, v, w, i, jg, pacc, nullptr, pol_in, pol_out);
+            __syncthreads();
+            if (tid == 0) {
+                __threadfence();
+                st_release_i32(&done[tk], 1);
+            }
+        }
+        const int sc = tk - lag;
+        unsigned long long best = 0ull;
+        if (sc >= 0) {
+            int i, jg;
+            k6_item_to_ij(sc, P.nx, ngrp, i, jg);
+            if (tid < 5) {   // the items that wrote what this step reads
+                const int di = (tid & 1) ? i + 1 : i;
+                const int dg = (tid == 4) ? 0 : ((tid & 2) ? jg - 1 : jg);
+                const bool need = (di < P.nx) && (dg >= 0) && (tid < 4 || (jg == ngrp - 1 && di == i));
+                if (need) {
+                    const int* f = &done[k6_ij_to_item(di, dg, P.nx, ngrp)];
+                    while (ld_acquire_i32(f) == 0) __nanosleep(64);
+                }
+            }
+            __syncthreads();
+            const int npass = (jg == ngrp - 1) ? 2 : 1;   // (the last group also takes line ny - 1)
+#pragma unroll 1
+            for (int pass = 0; pass < npass; ++pass) {
+                const int j = (pass == 0) ? jg * JL - 1 + (int)threadIdx.y : ((threadIdx.y == 0) ? P.ny - 1 : -1);
+                if (j >= 0) best = umax64(best, cfl_line<true>(P, u, v, w, i, j));
+            }
+        }
+        cfl_block_max(best, s_max, cfl);
+        __syncthreads();   // s_tk and s_max are rewritten by the next step
     }
 }
 

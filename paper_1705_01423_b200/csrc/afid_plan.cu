@@ -270,6 +270,9 @@ struct afid_plan {
     size_t ws_bytes;
     LaunchCfg k1, k2, k4, k5, k3;
     bool accumulate;   // p += phi instead of p = phi (afid_plan_set_accumulate)
+    int* cfl_sync;     // afid_project_cfl: ticket counter + one "corrected" flag per K6 item (device)
+    size_t cfl_sync_bytes;
+    int cfl_ctas;      // resident CTAs of k_correct_cfl
     int k3_kw;         // systems per K3 CTA (8 or 4)
     alignas(64) CUtensorMap mapC;   // K3's gather of C = ws[1] viewed as [nzh][nx][2 ny] doubles
     alignas(64) CUtensorMap mapD;   // K5's gather of D = ws[1], same view, 128-byte swizzle
@@ -346,6 +349,7 @@ static void discard_plan(afid_plan* pl)
     cudaFree(pl->ws[0]);
     cudaFree(pl->ws[1]);
     cudaFree(pl->tables);
+    cudaFree(pl->cfl_sync);
     delete pl;
 }
 
@@ -470,6 +474,19 @@ static afid_plan* create_impl(int nx, int ny, int nz, const double* xc, double L
             cudaGetLastError();
             discard_plan(pl); fail(AFID_ERR_NOMEM, "cudaMalloc(work arrays) failed"); return nullptr;
         }
+    {   // afid_project_cfl: flags and the persistent grid of the fused correction + CFL kernel
+        pl->cfl_sync_bytes = (1 + (size_t)nxl * (ny / K6_JL)) * sizeof(int);
+        if (cudaMalloc((void**)&pl->cfl_sync, pl->cfl_sync_bytes) != cudaSuccess) {
+            cudaGetLastError();
+            discard_plan(pl); fail(AFID_ERR_NOMEM, "cudaMalloc(cfl flags) failed"); return nullptr;
+        }
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)k_correct_cfl, K6_JL * K6_TX, 0) != cudaSuccess || occ < 1) {
+            cudaGetLastError();
+            discard_plan(pl); fail(AFID_ERR_CUDA, "k_correct_cfl does not fit an SM"); return nullptr;
+        }
+        pl->cfl_ctas = occ * pl->n_sm;
+    }
     if (!make_map3(&pl->mapC, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)nx, (uint64_t)nkz, 2 * (uint32_t)pl->k3_kw, (uint32_t)k3_box_rows(nx), 1,
                    CU_TENSOR_MAP_SWIZZLE_NONE)) {
         discard_plan(pl);
@@ -640,6 +657,22 @@ static int launch_correct(afid_plan* pl, double* u, double* v, double* w, double
     return AFID_OK;
 }
 
+// the fused correction + CFL maximum (afid_project_cfl): zero the ticket / flags, floor into *cfl, one persistent launch
+static int launch_correct_cfl(afid_plan* pl, double* u, double* v, double* w, double* p, cudaStream_t st, double* pacc, double* cfl)
+{
+    cudaError_t e = cudaMemsetAsync(pl->cfl_sync, 0, pl->cfl_sync_bytes, st);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(e));
+    k_cfl_init<<<1, 1, 0, st>>>(cfl);
+    const long long nitems = (long long)pl->nx * (pl->ny / K6_JL);
+    const int grid = (int)(nitems < pl->cfl_ctas ? nitems : pl->cfl_ctas);
+    int lag = grid + 16;
+    int* sync = pl->cfl_sync;
+    void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, (void*)&pacc, (void*)&cfl, (void*)&sync, &lag};
+    e = cudaLaunchKernel((const void*)k_correct_cfl, dim3((unsigned)grid), dim3(K6_TX, K6_JL), args, 0, st);
+    if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_correct_cfl: ") + cudaGetErrorString(e));
+    return AFID_OK;
+}
+
 // fork the auxiliary streams off `st` / join them back (both capturable in a CUDA graph)
 static int pipe_fork(afid_plan* pl, cudaStream_t st, int ns)
 {
@@ -692,7 +725,7 @@ static int run_solve(afid_plan* pl, cplx* outT, cudaStream_t st)
 
 // K4 + K5 + K6: T -> D -> p, u, v, w
 static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double* v, double* w, double* p, cudaStream_t st,
-                       cudaEvent_t ev_a, cudaEvent_t ev_b)
+                       cudaEvent_t ev_a, cudaEvent_t ev_b, double* cfl = nullptr)
 {
     int rc;
     // accumulate mode: phi goes to the (now dead) T work array, K6 corrects from it and adds it to p
@@ -703,8 +736,10 @@ static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double*
         if (ev_a && (rc = record(ev_a, st))) return rc;
         if ((rc = launch_k5(pl, phi, 0, pl->nx, pl->nx, st))) return rc;
         if (ev_b && (rc = record(ev_b, st))) return rc;
+        if (cfl) return launch_correct_cfl(pl, u, v, w, phi, st, pacc, cfl);
         return launch_correct(pl, u, v, w, phi, 0, pl->nx, st, pacc);
     }
+    if (cfl) return fail(AFID_ERR_UNSUPPORTED_SIZE, "afid_project_cfl: not available with plane-pipelined sweeps");
     // plane-pipelined: K4 of batch b (stream 0), K5 of batch b-1 (stream 1) and K6 of batch b-2 (stream 2)
     // overlap; D is a rotating buffer of `rot` batches, p is read back by K6 right after K5 wrote it
     const int nb = pl->pipe_batch, rot = pl->pipe_rot, dmod = nb * rot;
@@ -725,7 +760,7 @@ static int run_inverse(afid_plan* pl, const cplx* T, cplx* D, double* u, double*
 
 extern "C" {
 
-AFID_EXPORT int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void* stream)
+static int project_impl(afid_plan* pl, double* u, double* v, double* w, double* p, double* cfl, void* stream)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
     int rc;
@@ -741,12 +776,24 @@ AFID_EXPORT int afid_project(afid_plan* pl, double* u, double* v, double* w, dou
     if (tm && (rc = record(pl->ev[2], st))) return rc;
     if ((rc = run_solve(pl, pl->ws[0], st))) return rc;             // T in ws0
     if (tm && (rc = record(pl->ev[3], st))) return rc;
-    if ((rc = run_inverse(pl, pl->ws[0], pl->ws[1], u, v, w, p, st, tm ? pl->ev[4] : nullptr, tm ? pl->ev[5] : nullptr))) return rc;
+    if ((rc = run_inverse(pl, pl->ws[0], pl->ws[1], u, v, w, p, st, tm ? pl->ev[4] : nullptr, tm ? pl->ev[5] : nullptr, cfl))) return rc;
     if (tm) {
         if ((rc = record(pl->ev[6], st))) return rc;
         pl->ev_valid = true;
     }
     return AFID_OK;
+}
+
+AFID_EXPORT int afid_project(afid_plan* pl, double* u, double* v, double* w, double* p, void* stream)
+{
+    return project_impl(pl, u, v, w, p, nullptr, stream);
+}
+
+AFID_EXPORT int afid_project_cfl(afid_plan* pl, double* u, double* v, double* w, double* p, double* cfl, void* stream)
+{
+    if (!cfl) return fail(AFID_ERR_NULL, "cfl is NULL");
+    if (((size_t)cfl & 7) != 0) return fail(AFID_ERR_ALIGN, "cfl is not 8-byte aligned");
+    return project_impl(pl, u, v, w, p, cfl, stream);
 }
 
 // ---- the projection sharded over ranks (one process per GPU) -----------------------------------

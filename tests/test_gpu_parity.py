@@ -165,6 +165,52 @@ def test_max_cfl_parity(ov):
     plan.destroy()
 
 
+@pytest.mark.parametrize("ov", [SHAPES[1], SHAPES[4], SHAPES[7], dict(nx=256, ny=256, nz=256, grid="tanh", s=3.0),
+                                dict(nx=40, ny=8, nz=16), dict(nx=3, ny=40, nz=1280), dict(nx=130, ny=768, nz=64, grid="tanh", s=3.0)],
+                         ids=lambda o: f"{o['nx']}x{o['ny']}x{o['nz']}")
+def test_project_cfl_fused(ov):
+    """afid_project_cfl (fused form): u, v, w, p bit-identical to afid_project's; the CFL number
+    bit-identical to afid_max_cfl on the projected field (a maximum over the same per-cell values) and within
+    2e-15 of the oracle's Listing 1 on the oracle's projected field (the oracle's field differs from the GPU's
+    by the parity tolerance, so that comparison carries 1e-11); repeated calls (flags re-zeroed) agree; the
+    accumulate mode goes through the same kernel."""
+    cfg = synth.config("C1", **ov)
+    xc = synth.grid_faces(cfg)
+    nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
+    u, v, w = synth.velocity(cfg, xc)
+    plan = afid.Plan(nx, ny, nz, xc, cfg["Ly"], cfg["Lz"])
+    a = [t.cuda() for t in (u, v, w)]
+    b = [t.cuda() for t in (u, v, w)]
+    pa, pb = torch.empty_like(a[1]), torch.empty_like(a[1])
+    plan.project(*a, pa)
+    sep = float(plan.max_cfl(*a).cpu())
+    for rep in range(2):
+        for t, src in zip(b, (u, v, w)):
+            t.copy_(src)
+        pb.fill_(float("nan"))
+        fused = float(plan.project_cfl(*b, pb).cpu())
+        for x, y in zip(a + [pa], b + [pb]):
+            assert torch.equal(x, y)
+        assert fused == sep, (fused, sep)
+    if nx * ny * nz <= 2_000_000:   # (the naive-DFT oracle projection of 256^3 is covered by test_c2)
+        uo, vo, wo, po, _ = ref.project(xc, cfg["Ly"], cfg["Lz"], u.numpy(), v.numpy(), w.numpy())
+        want = ref.max_cfl(xc, cfg["Ly"], cfg["Lz"], uo, vo, wo)
+        assert abs(fused - want) <= 1e-11 * want, (fused, want)
+    want_gpu_field = ref.max_cfl(xc, cfg["Ly"], cfg["Lz"], a[0].cpu().numpy(), a[1].cpu().numpy(), a[2].cpu().numpy())
+    assert abs(fused - want_gpu_field) <= 2e-15 * want_gpu_field, (fused, want_gpu_field)
+    # accumulate mode: p += phi through the fused kernel
+    plan.set_accumulate(True)
+    for t, src in zip(b, (u, v, w)):
+        t.copy_(src)
+    pc = torch.ones_like(pb)
+    fused2 = float(plan.project_cfl(*b, pc).cpu())
+    assert fused2 == sep
+    assert torch.equal(b[0], a[0]) and torch.equal(b[1], a[1]) and torch.equal(b[2], a[2])
+    assert rel(pc.cpu().numpy(), 1.0 + pa.cpu().numpy()) <= 1e-15
+    plan.set_accumulate(False)
+    plan.destroy()
+
+
 @pytest.mark.parametrize("shape", [(5, 8, 16), (33, 24, 48), (64, 32, 64), (100, 16, 32), (256, 64, 64), (1030, 8, 32), (1024, 16, 64), (2048, 8, 32), (1700, 8, 16)],
                          ids=lambda t: "x".join(map(str, t)))
 def test_xsolve_parity(shape):
