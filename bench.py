@@ -76,18 +76,48 @@ def measured_peaks():
         return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
 
 
-def ncu_traffic(kernel):
-    """DRAM bytes per launch of `kernel` at C4 from the committed ncu capture, or None."""
-    path = os.path.join(ROOT, "profiles", "r1_c4_dram_traffic.csv")
+def built_kernel_names():
+    """Mangled names of the kernels in the built library (cuobjdump), or None if they cannot be listed."""
+    lib = os.path.join(ROOT, "paper_1705_01423_b200", "libafid_b200.so")
+    try:
+        out = subprocess.run(["cuobjdump", "--dump-resource-usage", lib], capture_output=True, text=True, timeout=60).stdout
+    except Exception:
+        return None
+    names = {ln.split("Function", 1)[1].strip().rstrip(":") for ln in out.splitlines() if ln.strip().startswith("Function")}
+    return names or None
+
+
+def ncu_traffic(kernel, ny, nz, nx, points):
+    """DRAM bytes per launch of `kernel` on this workload, scaled from the committed ncu capture
+    (profiles/r2_dram_traffic.csv: bytes per point on a slab with the same cross-section), or None when there is
+    no capture of that shape or the captured kernel (by mangled name) is no longer the one in the built library."""
+    path = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
     try:
         with open(path) as f:
-            for ln in f:
-                parts = ln.strip().split(",")
-                if parts and parts[0] == kernel:
-                    return float(parts[1]) + float(parts[2])
+            rows = [ln.strip().split(",") for ln in f if ln.strip()]
     except Exception:
-        pass
-    return None
+        return None, None
+    hdr = rows[0]
+    for r in rows[1:]:
+        d = dict(zip(hdr, r))
+        if d["kernel"] != kernel:
+            continue
+        sx, sy, sz = (int(x) for x in d["shape"].split("x"))
+        same = (sx == nx and sy == ny) if kernel == "k_solve_x" else (sy == ny and sz == nz)
+        if not same:
+            return None, "no capture of this shape"
+        names = built_kernel_names()
+        if names is None or d["mangled_name"] not in names:
+            return None, "captured kernel is not in the built library any more (or cuobjdump unavailable)"
+        return float(d["bytes_per_point"]) * points, f"profiles/r2_dram_traffic.csv (ncu at commit {d['commit']}, {d['shape']} slab, scaled by points)"
+    return None, None
+
+
+def git_sha():
+    try:
+        return subprocess.run(["git", "-C", ROOT, "rev-parse", "--short", "HEAD"], capture_output=True, text=True, timeout=10).stdout.strip() or None
+    except Exception:
+        return None
 
 
 class ClockSampler:
@@ -153,6 +183,9 @@ def run_gpu(args):
         dist.init_process_group("nccl", device_id=dev)
 
     cfg = synth.config(args.workload)
+    if args.shape:   # a slab / another shape with the workload's grid law and field recipe (profiling under ncu)
+        sx, sy, sz = (int(x) for x in args.shape.split(","))
+        cfg = synth.config(args.workload, nx=sx, ny=sy, nz=sz)
     nx, ny, nz = cfg["nx"], cfg["ny"], cfg["nz"]
     N = nx * ny * nz
     xc = synth.grid_faces(cfg)
@@ -253,29 +286,31 @@ def run_gpu(args):
             return t0.elapsed_time(t1) / reps
         out = torch.empty(1, dtype=torch.float64, device=dev)
         ms_cfl = timed(lambda: plan.max_cfl(u, v, w, out))
+        ms_pcfl = timed(lambda: plan.project_cfl(u, v, w, p, out), reps=3) if args.fused_cfl else None
         dxs = np.diff(xc)
         xs = plan.xsolve(np.r_[0.0, 1.0 / dxs[1:] ** 2], np.r_[1.0 / dxs[:-1] ** 2, 0.0], np.full(nx, 1.0e3))
         ms_xs = timed(lambda: xs.apply(p))
         xs.destroy()
-        extras = {"afid_max_cfl": {"ms": ms_cfl, "alg_GBps": 24.0 * N / (ms_cfl * 1e-3) / 1e9, "frac_of_peak": 24.0 * N / (ms_cfl * 1e-3) / 1e9 / peak},
+        extras = {"afid_project_cfl": ({"ms": ms_pcfl, "ms_over_afid_project": ms_pcfl - ms_local / args.steps} if ms_pcfl else "not timed (--fused-cfl)"),
+                  "afid_max_cfl": {"ms": ms_cfl, "alg_GBps": 24.0 * N / (ms_cfl * 1e-3) / 1e9, "frac_of_peak": 24.0 * N / (ms_cfl * 1e-3) / 1e9 / peak},
                   "afid_xsolve_apply": {"ms": ms_xs, "alg_GBps": 16.0 * N / (ms_xs * 1e-3) / 1e9, "frac_of_peak": 16.0 * N / (ms_xs * 1e-3) / 1e9 / peak}}
     except Exception as ex:
         extras = {"error": str(ex)[:200]}
     dom = max(kt, key=kt.get)
     ach = ALG_BYTES_PER_POINT[dom] * N / (kt[dom] * 1e-3) / 1e9
-    traffic = ncu_traffic(dom) if args.workload == "C4" else None
+    traffic, traffic_src = ncu_traffic(dom, ny, nz, nx, N)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": traffic, "peak_source": peak_src,
+                "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                 "alg_bytes_per_launch": ALG_BYTES_PER_POINT[dom] * N, "kernel_ms": kt[dom]}
     ms_step = ms_total / args.steps
     path_gbs = PATH_ALG_BYTES_PER_POINT * N / (ms_local / args.steps * 1e-3) / 1e9
     kernels = {k: {"ms": t, "alg_GBps": ALG_BYTES_PER_POINT[k] * N / (t * 1e-3) / 1e9,
                    "frac_of_peak": ALG_BYTES_PER_POINT[k] * N / (t * 1e-3) / 1e9 / peak} for k, t in kt.items()}
-    config = {"workload": f"{args.workload}: {nx}x{ny}x{nz} {cfg['grid']}-clustered x grid, Ly={cfg['Ly']:.6g}, "
+    config = {"workload": f"{args.workload}{' (--shape)' if args.shape else ''}: {nx}x{ny}x{nz} {cfg['grid']}-clustered x grid, Ly={cfg['Ly']:.6g}, "
                           f"Lz={cfg['Lz']:.6g}, seeded random-mode velocity (synth.py)",
               "points_per_step_per_gpu": N, "parallelism": "replicas only" if world > 1 else "1 gpu",
               "l2": "working set (>= 77 GB) far larger than the 126 MB L2; no flush needed",
-              "device_bytes": plan.workspace_bytes + (4 * N + ny * nz) * 8}
+              "device_bytes": plan.workspace_bytes + (4 * N + ny * nz) * 8, "git_sha": git_sha()}
     line = make_line(config, world, args.steps, args.warmup, ms_total, pts, clocks=clocks, e2e=e2e,
                      gpu_launches=plan.num_launches * args.steps, roofline=roofline, kernels=kernels, extras=extras,
                      path_roofline={"alg_bytes_per_point": PATH_ALG_BYTES_PER_POINT, "achieved_GBps": path_gbs,
@@ -379,11 +414,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--shape", default=None, help="nx,ny,nz: time this shape with the workload's grid law and field recipe "
+                                                  "(slabs for ncu captures; the headline is the unmodified workload)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--pipeline", default=None, help="planes_per_batch,rotation (afid_plan_set_pipeline)")
     ap.add_argument("--hints", type=int, default=None, help="L2 hint mask (afid_plan_set_l2_hints)")
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--fused-cfl", action="store_true", help="also time afid_project_cfl (SURVEY.md 8(f3), fused form) in the extras")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     maybe_spawn_ranks(args)
