@@ -149,6 +149,8 @@ int afid_xsolve_destroy(afid_xsolve* h);
  * afid_plan_set_l2_hints -- bit mask of L2 eviction-priority hints the kernels attach to their accesses:
  *   1 streamed loads (u, v, w, spectra read once) evict-first      2 intermediates (B, D) evict-last
  *   4 loads of the intermediates evict-first                       8 streamed stores evict-first
+ *   32 afid_project_cfl runs its two-CTAs-per-SM kernel variant (in that kernel bit 2 also makes the corrected
+ *      lines evict-last and bit 4 drops the evict-first hint of the uncorrected loads): measurement switches
  * Default 0.  Hints change timing only, never results.
  */
 int afid_plan_set_pipeline(afid_plan* plan, int planes_per_batch, int rotation);

@@ -443,11 +443,13 @@ __global__ void __launch_bounds__(LPR* PL::TPL, 1) k_c2r_z(DevParams P, const __
 constexpr int K6_JL = 4, K6_TX = 64, K6_U = 4;
 
 // the correction of the lines (i, JL jg .. JL jg + JL - 1); called by all K6_JL x K6_TX threads of a CTA
+// (U = cell pairs per thread and load batch)
+template <int U>
 __device__ __forceinline__ void k6_correct_item(const DevParams& P, const double* __restrict__ p, double* __restrict__ u, double* __restrict__ v,
                                                 double* __restrict__ w, int i, int jg, double* __restrict__ pacc, const double* __restrict__ p_halo,
                                                 unsigned long long pol_in, unsigned long long pol_out)
 {
-    constexpr int JL = K6_JL, TX = K6_TX, U = K6_U;
+    constexpr int JL = K6_JL, TX = K6_TX;
     const int j = jg * JL + threadIdx.y;
     const int jm = (j == 0) ? P.ny - 1 : j - 1;
     const size_t plane = (size_t)P.ny * P.nz;
@@ -531,7 +533,7 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct(DevParams P, const dou
     // this launch covers planes i_base .. i_base+np-1.
     int i, jg;
     k6_item_to_ij((int)blockIdx.x, np, P.ny / K6_JL, i, jg);
-    k6_correct_item(P, p, u, v, w, i_base + i, jg, pacc, p_halo, l2_policy((P.hints & 1) ? 1 : 0), l2_policy((P.hints & 8) ? 1 : 0));
+    k6_correct_item<K6_U>(P, p, u, v, w, i_base + i, jg, pacc, p_halo, l2_policy((P.hints & 1) ? 1 : 0), l2_policy((P.hints & 8) ? 1 : 0));
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1004,11 +1006,11 @@ __device__ __forceinline__ double ldcg1(const double* p)
 // Listing 1 over the cells of ONE line (i, j, all k) per thread row: thread x takes the cell pairs kp = x, x + TX, ...
 // in batches of U.  Returns the bit pattern of the thread's maximum.  CG: the loads bypass L1 (the fused kernel reads
 // what other SMs wrote a moment ago; L1 may still hold the uncorrected lines).
-template <bool CG>
+template <bool CG, int U>
 __device__ __forceinline__ unsigned long long cfl_line(const DevParams& P, const double* __restrict__ u, const double* __restrict__ v,
                                                        const double* __restrict__ w, int i, int j)
 {
-    constexpr int TX = K6_TX, U = K6_U;
+    constexpr int TX = K6_TX;
     const int jp = (j + 1 == P.ny) ? 0 : j + 1;
     const size_t plane = (size_t)P.ny * P.nz;
     const size_t ol = ((size_t)i * P.ny + j) * P.nz;
@@ -1066,7 +1068,7 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_max_cfl(DevParams P, const dou
     __shared__ unsigned long long s_max[K6_JL * K6_TX / 32];
     int i, jg;
     k6_item_to_ij((int)blockIdx.x, P.nx, P.ny / K6_JL, i, jg);
-    cfl_block_max(cfl_line<false>(P, u, v, w, i, jg * K6_JL + threadIdx.y), s_max, cfl);
+    cfl_block_max(cfl_line<false, K6_U>(P, u, v, w, i, jg * K6_JL + threadIdx.y), s_max, cfl);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1090,7 +1092,10 @@ __device__ __forceinline__ int ld_acquire_i32(const int* p)
 }
 __device__ __forceinline__ void st_release_i32(int* p, int v) { asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory"); }
 
-__global__ void __launch_bounds__(K6_JL* K6_TX) k_correct_cfl(DevParams P, const double* __restrict__ p, double* __restrict__ u, double* __restrict__ v,
+// U, MINB: cell pairs per load batch and CTAs per SM the register allocation is capped for.  <4, 1> (236 registers, one
+// CTA per SM) is the measured default; <2, 2> lets one CTA's reduce step overlap the other's correction (hint bit 32).
+template <int U, int MINB>
+__global__ void __launch_bounds__(K6_JL* K6_TX, MINB) k_correct_cfl(DevParams P, const double* __restrict__ p, double* __restrict__ u, double* __restrict__ v,
                                                               double* __restrict__ w, double* __restrict__ pacc, double* __restrict__ cfl, int* __restrict__ sync,
                                                               int lag)
 {
@@ -1100,7 +1105,8 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct_cfl(DevParams P, const
     const int tid = threadIdx.y * TX + threadIdx.x;
     const int ngrp = P.ny / JL, nitems = P.nx * ngrp;
     int* done = sync + 1;
-    const unsigned long long pol_in = l2_policy((P.hints & 4) ? 0 : 1), pol_out = l2_policy((P.hints & 2) ? 2 : 0);   // the uncorrected u, v, w are read once: evict first
+    // the uncorrected u, v, w are read once: evict first; hint bit 2: the corrected lines evict last (kept for the reduce step)
+    const unsigned long long pol_in = l2_policy((P.hints & 4) ? 0 : 1), pol_out = l2_policy((P.hints & 2) ? 2 : 0);
     int nxt = 0;
     if (tid == 0) nxt = atomicAdd(&sync[0], 1);
 #pragma unroll 1
@@ -1115,7 +1121,7 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct_cfl(DevParams P, const
         if (tk < nitems) {
             int i, jg;
             k6_item_to_ij(tk, P.nx, ngrp, i, jg);
-            k6_correct_item(P, p, u, v, w, i, jg, pacc, nullptr, pol_in, pol_out);
+            k6_correct_item<U>(P, p, u, v, w, i, jg, pacc, nullptr, pol_in, pol_out);
             __syncthreads();
             if (tid == 0) {
                 __threadfence();
@@ -1141,7 +1147,7 @@ __global__ void __launch_bounds__(K6_JL* K6_TX) k_correct_cfl(DevParams P, const
 #pragma unroll 1
             for (int pass = 0; pass < npass; ++pass) {
                 const int j = (pass == 0) ? jg * JL - 1 + (int)threadIdx.y : ((threadIdx.y == 0) ? P.ny - 1 : -1);
-                if (j >= 0) best = umax64(best, cfl_line<true>(P, u, v, w, i, j));
+                if (j >= 0) best = umax64(best, cfl_line<true, U>(P, u, v, w, i, j));
             }
         }
         cfl_block_max(best, s_max, cfl);

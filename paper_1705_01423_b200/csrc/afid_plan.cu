@@ -272,7 +272,8 @@ struct afid_plan {
     bool accumulate;   // p += phi instead of p = phi (afid_plan_set_accumulate)
     int* cfl_sync;     // afid_project_cfl: ticket counter + one "corrected" flag per K6 item (device)
     size_t cfl_sync_bytes;
-    int cfl_ctas;      // resident CTAs of k_correct_cfl
+    int cfl_ctas;      // resident CTAs of k_correct_cfl<K6_U, 1>
+    int cfl_ctas2;     // ... of the <2, 2> variant (hint bit 32)
     int k3_kw;         // systems per K3 CTA (8 or 4)
     alignas(64) CUtensorMap mapC;   // K3's gather of C = ws[1] viewed as [nzh][nx][2 ny] doubles
     alignas(64) CUtensorMap mapD;   // K5's gather of D = ws[1], same view, 128-byte swizzle
@@ -480,12 +481,14 @@ static afid_plan* create_impl(int nx, int ny, int nz, const double* xc, double L
             cudaGetLastError();
             discard_plan(pl); fail(AFID_ERR_NOMEM, "cudaMalloc(cfl flags) failed"); return nullptr;
         }
-        int occ = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)k_correct_cfl, K6_JL * K6_TX, 0) != cudaSuccess || occ < 1) {
+        int occ = 0, occ2 = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)k_correct_cfl<K6_U, 1>, K6_JL * K6_TX, 0) != cudaSuccess || occ < 1 ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, (const void*)k_correct_cfl<2, 2>, K6_JL * K6_TX, 0) != cudaSuccess || occ2 < 1) {
             cudaGetLastError();
             discard_plan(pl); fail(AFID_ERR_CUDA, "k_correct_cfl does not fit an SM"); return nullptr;
         }
         pl->cfl_ctas = occ * pl->n_sm;
+        pl->cfl_ctas2 = occ2 * pl->n_sm;
     }
     if (!make_map3(&pl->mapC, pl->ws[1], 2 * (uint64_t)ny, (uint64_t)nx, (uint64_t)nkz, 2 * (uint32_t)pl->k3_kw, (uint32_t)k3_box_rows(nx), 1,
                    CU_TENSOR_MAP_SWIZZLE_NONE)) {
@@ -562,7 +565,7 @@ AFID_EXPORT int afid_plan_num_launches(const afid_plan* pl)
 AFID_EXPORT int afid_plan_set_l2_hints(afid_plan* pl, int mask)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");
-    if (mask < 0 || mask > 15) return fail(AFID_ERR_UNSUPPORTED_SIZE, "hint mask must be in [0, 15]");
+    if (mask < 0 || mask > 63) return fail(AFID_ERR_UNSUPPORTED_SIZE, "hint mask must be in [0, 63]");
     pl->dp.hints = mask;
     return AFID_OK;
 }
@@ -664,11 +667,13 @@ static int launch_correct_cfl(afid_plan* pl, double* u, double* v, double* w, do
     if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("cudaMemsetAsync: ") + cudaGetErrorString(e));
     k_cfl_init<<<1, 1, 0, st>>>(cfl);
     const long long nitems = (long long)pl->nx * (pl->ny / K6_JL);
-    const int grid = (int)(nitems < pl->cfl_ctas ? nitems : pl->cfl_ctas);
+    const bool v2 = (pl->dp.hints & 32) != 0;
+    const int ctas = v2 ? pl->cfl_ctas2 : pl->cfl_ctas;
+    const int grid = (int)(nitems < ctas ? nitems : ctas);
     int lag = grid + 16;
     int* sync = pl->cfl_sync;
     void* args[] = {&pl->dp, (void*)&p, (void*)&u, (void*)&v, (void*)&w, (void*)&pacc, (void*)&cfl, (void*)&sync, &lag};
-    e = cudaLaunchKernel((const void*)k_correct_cfl, dim3((unsigned)grid), dim3(K6_TX, K6_JL), args, 0, st);
+    e = cudaLaunchKernel(v2 ? (const void*)k_correct_cfl<2, 2> : (const void*)k_correct_cfl<K6_U, 1>, dim3((unsigned)grid), dim3(K6_TX, K6_JL), args, 0, st);
     if (e != cudaSuccess) return fail(AFID_ERR_CUDA, std::string("k_correct_cfl: ") + cudaGetErrorString(e));
     return AFID_OK;
 }
