@@ -160,3 +160,21 @@ def test_shard_bounds_partition():
         assert max(hi - lo for lo, hi in b) - min(hi - lo for lo, hi in b) <= 1
     with pytest.raises(afid.AfidError):
         afid.shard_bounds(3, 4, 0)
+
+
+def test_bench_traffic_comes_only_from_a_matching_capture(built_lib):
+    """bench.py's roofline.traffic is the committed ncu capture's DRAM bytes per point scaled to the workload; it is
+    withheld when the capture has another cross-section or when the captured kernel (by mangled name) is no longer the
+    one in the built library."""
+    import shutil
+    sys.path.insert(0, ROOT)
+    import bench
+    n = 1024 * 1536 * 1536
+    t, src = bench.ncu_traffic("k_correct", 1536, 1536, 1024, n)
+    if shutil.which("cuobjdump") is None:
+        assert t is None
+    else:
+        assert t is not None and 55.0 <= t / n <= 57.0 and "r2_dram_traffic.csv" in src   # algorithmic 56 B/pt
+    assert bench.ncu_traffic("k_correct", 1024, 1024, 512, 1)[0] is None                  # another cross-section
+    assert bench.ncu_traffic("k_c2r_z", 1536, 1536, 1024, n)[0] is None                   # kernel changed since the capture
+    assert bench.ncu_traffic("no_such_kernel", 1536, 1536, 1024, n) == (None, None)
