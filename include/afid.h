@@ -104,6 +104,11 @@ int afid_max_cfl(afid_plan* plan, const double* u, const double* v, const double
  * graph.  Unsharded plans only; not available with afid_plan_set_pipeline.
  */
 int afid_project_cfl(afid_plan* plan, double* u, double* v, double* w, double* p, double* cfl, void* stream);
+/* afid_cfl_schedule -- HOST arithmetic only (no device, no plan), for tests of the fused launch's schedule: ticket t
+ * corrects item t = lines 4 jg .. 4 jg + 3 of plane i (the order of the correction kernel) and then reduces the
+ * cells of item t - lag, lines [line_lo, line_hi] (one line down) plus extra_line (ny - 1 for the last group, else
+ * -1), after the items deps[0..4] (-1 = none) have been corrected.  ny must be a multiple of 4. */
+int afid_cfl_schedule(int nx, int ny, int item, int* i, int* jg, int* line_lo, int* line_hi, int* extra_line, int* deps);
 
 /*
  * afid_plan_set_accumulate -- SURVEY.md 8(f3): choose what afid_project does with p.

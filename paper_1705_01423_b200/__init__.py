@@ -23,7 +23,7 @@ SYMBOLS = ["afid_plan_create", "afid_project", "afid_plan_destroy", "afid_plan_w
            "afid_plan_num_launches", "afid_stage_forward", "afid_stage_solve", "afid_fft_length_supported",
            "afid_max_nx", "afid_last_error", "afid_last_error_code", "afid_version",
            "afid_plan_enable_timing", "afid_plan_kernel_times", "afid_plan_kernel_name",
-           "afid_fft_half_length_supported", "afid_max_cfl", "afid_project_cfl", "afid_plan_set_accumulate", "afid_xsolve_create", "afid_xsolve_apply",
+           "afid_fft_half_length_supported", "afid_max_cfl", "afid_project_cfl", "afid_cfl_schedule", "afid_plan_set_accumulate", "afid_xsolve_create", "afid_xsolve_apply",
            "afid_xsolve_destroy", "afid_plan_set_pipeline", "afid_plan_set_l2_hints", "afid_plan_num_timed",
            "afid_shard_plan_create", "afid_shard_bounds", "afid_shard_layout", "afid_shard_buffers", "afid_shard_info",
            "afid_shard_forward", "afid_shard_solve", "afid_shard_inverse", "afid_shard_correct"]
@@ -68,6 +68,8 @@ def lib():
         L.afid_xsolve_destroy.argtypes = [vp]
         L.afid_plan_set_accumulate.restype = i
         L.afid_plan_set_accumulate.argtypes = [vp, i]
+        L.afid_cfl_schedule.restype = i
+        L.afid_cfl_schedule.argtypes = [i, i, i, vp, vp, vp, vp, vp, vp]
         L.afid_project_cfl.restype = i
         L.afid_project_cfl.argtypes = [vp, vp, vp, vp, vp, vp, vp]
         L.afid_max_cfl.restype = i
@@ -290,6 +292,14 @@ class XSolve:
 # ------------------------------------------------------------------------------------------
 # the projection sharded over ranks (include/afid.h, afid_shard_*)
 # ------------------------------------------------------------------------------------------
+def cfl_schedule(nx, ny, item):
+    """afid_cfl_schedule (host arithmetic): (i, jg, line_lo, line_hi, extra_line, deps[5]) of item `item`."""
+    out = [C.c_int() for _ in range(5)]
+    deps = (C.c_int * 5)()
+    _check(lib().afid_cfl_schedule(int(nx), int(ny), int(item), *[C.byref(o) for o in out], deps))
+    return tuple(o.value for o in out) + (list(deps),)
+
+
 def shard_bounds(n, nranks, rank):
     """afid_shard_bounds: part `rank` of n items, [lo, hi) (host arithmetic, no device)."""
     lo, hi = C.c_int(0), C.c_int(0)

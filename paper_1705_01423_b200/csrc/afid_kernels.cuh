@@ -509,18 +509,18 @@ __device__ __forceinline__ void k6_correct_item(const DevParams& P, const double
 // item s of the CTA order of K6 -> (plane i, line group jg): j-chunks of JC groups outermost, then i, then the group inside
 // the chunk, so that plane i-1 of p (read again for the x-gradient) is still in L2 when plane i is processed
 constexpr int K6_JC = 32 / K6_JL;
-__device__ __forceinline__ void k6_item_to_ij(int s, int np, int ngrp, int& i, int& jg)
+__host__ __device__ __forceinline__ void k6_item_to_ij(int s, int np, int ngrp, int& i, int& jg)
 {
     const int per_chunk = np * K6_JC;
     const int chunk = s / per_chunk, rem = s % per_chunk;
-    const int jc_here = min(K6_JC, ngrp - chunk * K6_JC);
+    const int jc_here = (K6_JC < ngrp - chunk * K6_JC) ? K6_JC : ngrp - chunk * K6_JC;
     i = rem / jc_here;
     jg = chunk * K6_JC + rem % jc_here;
 }
-__device__ __forceinline__ int k6_ij_to_item(int i, int jg, int np, int ngrp)
+__host__ __device__ __forceinline__ int k6_ij_to_item(int i, int jg, int np, int ngrp)
 {
     const int chunk = jg / K6_JC;
-    const int jc_here = min(K6_JC, ngrp - chunk * K6_JC);
+    const int jc_here = (K6_JC < ngrp - chunk * K6_JC) ? K6_JC : ngrp - chunk * K6_JC;
     return chunk * np * K6_JC + i * jc_here + (jg - chunk * K6_JC);
 }
 

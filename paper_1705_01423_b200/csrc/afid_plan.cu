@@ -949,6 +949,28 @@ AFID_EXPORT int afid_max_cfl(afid_plan* pl, const double* u, const double* v, co
     return AFID_OK;
 }
 
+// Host arithmetic only (no device, no plan): the schedule of afid_project_cfl's fused launch, for tests.
+// Item `item` of the correction order = lines 4 jg .. 4 jg + 3 of plane i; its reduce step owns the lines
+// [line_lo, line_hi] (plus `extra_line` >= 0 for the last group) and waits for the items deps[0..4] (-1 = none).
+AFID_EXPORT int afid_cfl_schedule(int nx, int ny, int item, int* i, int* jg, int* line_lo, int* line_hi, int* extra_line, int* deps)
+{
+    if (nx < 1 || ny < K6_JL || (ny % K6_JL) != 0 || !i || !jg || !line_lo || !line_hi || !extra_line || !deps)
+        return fail(AFID_ERR_UNSUPPORTED_SIZE, "afid_cfl_schedule: bad arguments");
+    const int ngrp = ny / K6_JL;
+    if (item < 0 || item >= nx * ngrp) return fail(AFID_ERR_UNSUPPORTED_SIZE, "afid_cfl_schedule: item out of range");
+    k6_item_to_ij(item, nx, ngrp, *i, *jg);
+    *line_lo = (*jg == 0) ? 0 : *jg * K6_JL - 1;
+    *line_hi = *jg * K6_JL + K6_JL - 2;
+    *extra_line = (*jg == ngrp - 1) ? ny - 1 : -1;
+    for (int d = 0; d < 5; ++d) {   // the rule of k_correct_cfl's threads 0..4
+        const int di = (d & 1) ? *i + 1 : *i;
+        const int dg = (d == 4) ? 0 : ((d & 2) ? *jg - 1 : *jg);
+        const bool need = (di < nx) && (dg >= 0) && (d < 4 || (*jg == ngrp - 1 && di == *i));
+        deps[d] = need ? k6_ij_to_item(di, dg, nx, ngrp) : -1;
+    }
+    return AFID_OK;
+}
+
 AFID_EXPORT int afid_plan_set_accumulate(afid_plan* pl, int on)
 {
     if (!pl) return fail(AFID_ERR_NULL, "plan is NULL");

@@ -178,3 +178,39 @@ def test_bench_traffic_comes_only_from_a_matching_capture(built_lib):
     assert bench.ncu_traffic("k_correct", 1024, 1024, 512, 1)[0] is None                  # another cross-section
     assert bench.ncu_traffic("k_c2r_z", 1536, 1536, 1024, n)[0] is None                   # kernel changed since the capture
     assert bench.ncu_traffic("no_such_kernel", 1536, 1536, 1024, n) == (None, None)
+
+
+@pytest.mark.parametrize("nx,ny", [(1, 8), (3, 8), (5, 40), (7, 36), (64, 128), (9, 1536)])
+def test_fused_cfl_schedule_is_deadlock_free_and_covers_every_cell(built_lib, nx, ny):
+    """afid_project_cfl (fused form): ticket t corrects item t and then reduces item t - lag.  From the
+    library's own schedule arithmetic (afid_cfl_schedule, host only): the items are a bijection onto (plane, line
+    group); every dependency of a reduce step is an item at most 8 tickets after it (so with lag > 8 every wait is
+    for an EARLIER ticket: no deadlock for any CTA order); each dependency is exactly an item that owns a line the
+    step reads (lines lo..hi+1 of planes i and i+1, line 0 for the wrap); and the reduce steps of a plane cover
+    every line exactly once."""
+    import paper_1705_01423_b200 as afid
+    ngrp = ny // 4
+    seen, cover = set(), {}
+    for s in range(nx * ngrp):
+        i, jg, lo, hi, extra, deps = afid.cfl_schedule(nx, ny, s)
+        assert 0 <= i < nx and 0 <= jg < ngrp and (i, jg) not in seen
+        seen.add((i, jg))
+        lines = list(range(lo, hi + 1)) + ([extra] if extra >= 0 else [])
+        for j in lines:
+            assert (i, j) not in cover
+            cover[(i, j)] = s
+        need = set()                                   # owners of everything the cells (i, lines, :) read
+        for j in lines:
+            for (pi, pj) in ((i, j), (i + 1, j), (i, (j + 1) % ny)):
+                if pi < nx:                            # plane nx is the wall plane: never written
+                    need.add((pi, pj // 4))
+        got = set()
+        for d in deps:
+            if d >= 0:
+                assert d <= s + 8, (s, d)              # lag = resident CTAs + 16 > 8
+                di, dg = afid.cfl_schedule(nx, ny, d)[:2]
+                got.add((di, dg))
+        assert got == need, (s, got, need)
+    assert len(seen) == nx * ngrp and len(cover) == nx * ny
+    with pytest.raises(afid.AfidError):
+        afid.cfl_schedule(nx, ny, nx * ngrp)
