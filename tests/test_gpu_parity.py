@@ -360,6 +360,33 @@ def test_c2_full_parity():
     check_against_oracle(cfg, xc, u, v, w)
 
 
+def test_two_live_plans_of_different_nx_and_an_xsolve_handle():
+    """One kernel instantiation serves many nx and several live plans: the dynamic shared-memory limit of a function
+    is raised once and never lowered by a later, smaller plan.  Plan nx = 512 first, then nx = 384
+    (same k_solve_x instantiation, smaller tile) and an xsolve handle; the OLDER plan must still project."""
+    cfgs = [synth.config("C1", nx=512, ny=8, nz=16, grid="tanh", s=3.0), synth.config("C1", nx=384, ny=8, nz=16, grid="tanh", s=3.0)]
+    xcs = [synth.grid_faces(c) for c in cfgs]
+    plans = [afid.Plan(c["nx"], c["ny"], c["nz"], xc, c["Ly"], c["Lz"]) for c, xc in zip(cfgs, xcs)]
+    xs = plans[1].xsolve(np.full(384, 2.0), np.full(384, 3.0), np.full(384, 10.0))
+    for k in (0, 1, 0):                                    # the older plan first, and again after the newer one ran
+        cfg, xc, plan = cfgs[k], xcs[k], plans[k]
+        u, v, w = synth.velocity(cfg, xc)
+        uo, vo, wo, po, _ = ref.project(xc, cfg["Ly"], cfg["Lz"], u.numpy(), v.numpy(), w.numpy())
+        ud, vd, wd = u.cuda(), v.cuda(), w.cuda()
+        p = torch.empty_like(vd)
+        plan.project(ud, vd, wd, p)
+        torch.cuda.synchronize()
+        assert rel(p.cpu().numpy(), po) <= TOL and rel(ud.cpu().numpy(), uo) <= TOL
+        assert rel(vd.cpu().numpy(), vo) <= TOL and rel(wd.cpu().numpy(), wo) <= TOL
+    f = torch.ones((384, 8, 16), dtype=torch.float64, device="cuda")
+    xs.apply(f)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(f).all())
+    xs.destroy()
+    for pl in plans:
+        pl.destroy()
+
+
 def test_error_codes():
     xc = np.linspace(0.0, 1.0, 33)
     with pytest.raises(afid.AfidError) as e:
