@@ -317,6 +317,10 @@ def run_gpu(args):
                                     "frac_of_nominal_8TBs": path_gbs / NOMINAL_HBM_GBS, "frac_of_measured": path_gbs / peak})
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(args.workload)
+        try:
+            line["cpu_baseline_fft"] = cpu_baseline_fft(args.workload)
+        except Exception as ex:
+            line["cpu_baseline_fft"] = {"value": None, "error": str(ex)[:200]}
     elif rank == 0:
         line["cpu_baseline"] = None
     plan.destroy()
@@ -354,6 +358,27 @@ def cpu_baseline(workload):
     n = cfg["nx"] * cfg["ny"] * cfg["nz"]
     return {"value": n / dt / 1e6, "unit": UNIT, "cores": ref.num_threads(), "kind": "oracle",
             "sample": desc + f"; one oracle projection, {dt:.1f} s"}
+
+
+def cpu_baseline_fft(workload):
+    """The FFT form of the oracle (oracle/ref_fft.py: scipy.fft for the two DFTs, the C oracle's long-double Thomas,
+    divergence and correction) on a 32-plane slab of the workload's cross-section: the per-point cost of this form
+    does not depend on nx.  Reported next to cpu_baseline so that the line also has a CPU number for the
+    O(n log n) algorithm the paper's CPU code runs; it is a context figure, not a target."""
+    from oracle import ref, ref_fft
+    from paper_1705_01423_b200 import synth
+    full = synth.config(workload)
+    nxs = min(32, full["nx"])
+    cfg = synth.config(workload, nx=nxs)
+    xc = synth.grid_faces(full)[:nxs + 1].copy()
+    u, v, w = (t.numpy() for t in synth.velocity(cfg, xc))
+    t0 = time.perf_counter()
+    ref_fft.project_fft(xc, cfg["Ly"], cfg["Lz"], u, v, w)
+    dt = time.perf_counter() - t0
+    n = cfg["nx"] * cfg["ny"] * cfg["nz"]
+    return {"value": n / dt / 1e6, "unit": UNIT, "cores": ref.num_threads(), "kind": "oracle, FFT form (scipy.fft + long-double Thomas)",
+            "sample": f"{workload} cross-section slab: nx={nxs} x ny={cfg['ny']} x nz={cfg['nz']} (first {nxs} cells of the x grid); "
+                      f"one projection, {dt:.1f} s"}
 
 
 def run_reference(args):

@@ -373,6 +373,24 @@ def test_dense_large_case_oracle_matches_long_double_oracle():
     assert rel(pp, phi_m) <= 1e-12 and rel(uu, u_s) <= 1e-12 and rel(vv, v_s) <= 1e-12 and rel(ww, w_s) <= 1e-12
 
 
+def test_fft_form_oracle_matches_long_double_oracle():
+    """oracle/ref_fft.py (the two DFTs by scipy.fft, everything else the C oracle's routines; timed by bench.py as
+    cpu_baseline_fft) against the long-double naive-DFT definition: non-power-of-two and odd-factor lengths, non-uniform
+    grids, Ly != Lz, the mean-shear input."""
+    from oracle import ref_fft
+    for ov in (dict(nx=6, ny=12, nz=10), dict(nx=33, ny=40, nz=36, grid="tanh", s=3.0, Ly=1.3, Lz=0.7),
+               dict(nx=9, ny=30, nz=28, grid="erf", s=1.5, x_lo=-1.0, x_hi=1.0, Ly=3.0, Lz=0.7, shear=1.0, A=0.1)):
+        cfg = synth.config("C1", **ov)
+        xc = synth.grid_faces(cfg)
+        u, v, w = [t.numpy() for t in synth.velocity(cfg, xc)]
+        want = ref.project(xc, cfg["Ly"], cfg["Lz"], u, v, w)
+        uu, vv, ww = u.copy(), v.copy(), w.copy()
+        pp = ref_fft.project_fft(xc, cfg["Ly"], cfg["Lz"], uu, vv, ww)
+        for got, ref_ in zip((uu, vv, ww, pp), want[:4]):
+            assert rel(got, ref_) <= 1e-14
+        assert rel(uu - u, want[0] - u) <= 1e-13 and rel(vv - v, want[1] - v) <= 1e-13      # increments
+
+
 def test_oracle_header_says_test_infrastructure():
     here = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     txt = open(os.path.join(here, "oracle", "afid_ref.c")).read()
